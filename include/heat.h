@@ -1,0 +1,183 @@
+/*
+ * heat.h -- C-ABI boundary of the B200-native hot path of arXiv 1408.5853
+ * (Ayriyan, Busa Jr., Donets, Grigorian, Pribis: "Algorithm and Simulation of Heat
+ * Conduction Process for Design of a Thin Multilayer Technical Device").
+ *
+ * The library advances the paper's explicit-implicit finite-difference scheme, eq. (8)
+ * P:L108-113 ("P:Lnnn" = line of the paper text), one time step T -> T^ at a time:
+ *
+ *     rho c_V(T) (T^ - T)/tau = Lambda_i[T^] + Lambda_j[T] + X        (8)
+ *
+ * implicit in r (one tridiagonal system per z-line, eqs. (12)-(20) P:L131-192), explicit in
+ * z (eq. (11)), coefficients at the current level, no iterations.  All
+ * arithmetic is fp64 and runs in hand-written sm_100a CUDA kernels; there is no CPU path.
+ *
+ * Conventions
+ *   - i = radial node index 0..nr-1, j = axial node index 0..nz-1; node counts include the
+ *     boundary nodes (nr = N+1, nz = M+1 in the paper's ranges, eq. (9)).
+ *   - Field layout at this boundary: [batch][nz][nr], r fastest, fp64.
+ *   - "host" / "device" is stated for every pointer.  The library never allocates device
+ *     memory: the caller owns the two field levels, the workspace and the probe buffer and
+ *     must keep them alive until heat_destroy.  Small host arrays are copied at create time.
+ *   - Every call returns a heat_status; nothing throws or longjmps across the boundary.
+ *     A message for the last failure is available from heat_last_error.
+ *   - heat_step is asynchronous on the caller's stream; a CUDA fault raised by it surfaces
+ *     as HEAT_ECUDA from the next synchronising call (heat_get_field to host, heat_probe).
+ */
+#ifndef HEAT_B200_H
+#define HEAT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct heat_ctx heat_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    HEAT_OK = 0,
+    HEAT_EINVAL = 1, /* malformed descriptor / argument */
+    HEAT_ENOMEM = 2, /* workspace or probe buffer too small, host allocation failed */
+    HEAT_ECUDA = 3,  /* CUDA runtime error, no usable sm_100 device */
+    HEAT_ERANGE = 4  /* a property law is not strictly positive on the declared T range */
+} heat_status;
+
+/* Property law f(T).  The paper fits polynomials (23),(24) P:L245-248; BASELINE.json's
+ * workloads use power laws.
+ *   HEAT_LAW_CONST : f = c[0]
+ *   HEAT_LAW_POWER : f = c[0] * (T / T_ref)^c[1]
+ *   HEAT_LAW_POLY  : f = sum_{k=0..4} c[k] T^k   (ascending powers)                        */
+enum { HEAT_LAW_CONST = 0, HEAT_LAW_POWER = 1, HEAT_LAW_POLY = 2 };
+typedef struct {
+    int32_t kind;
+    int32_t reserved;
+    double c[5];
+    double T_ref;
+} heat_law;
+
+/* One material (the paper's index m, eq. (1)). */
+typedef struct {
+    heat_law k;         /* lambda_m(T), thermal conductivity                                 */
+    heat_law cp;        /* c_Vm(T), specific heat                                            */
+    double rho;         /* rho_m, density                                                    */
+    int32_t is_heater;  /* X_m != 0 only in flagged layers (2) P:L70                         */
+    int32_t reserved;
+    heat_law src_shape; /* s(T): X = Q0 * s(T) * nu(t) * p^2(t); chi(T) of (25) P:L274 up to
+                           a constant; CONST 1 for a temperature-independent source          */
+} heat_layer;
+
+/* Boundary condition of one side, (6) P:L90-95 generalised per side. */
+enum { HEAT_BC_NEUMANN0 = 0, HEAT_BC_DIRICHLET = 1 };
+typedef struct {
+    int32_t kind;
+    int32_t reserved;
+    double value; /* Dirichlet temperature */
+} heat_bc;
+
+#define HEAT_MAX_LAYERS 16
+#define HEAT_MAX_PROBES 64
+#define HEAT_MAX_NR 8192 /* one thread block owns a whole z-line */
+
+typedef struct {
+    int32_t nr, nz, batch, nlayers;  /* nr,nz >= 3; batch >= 1; 1 <= nlayers <= HEAT_MAX_LAYERS */
+    const double *r;                 /* host, nr, strictly ascending, r[0] >= 0 (9) P:L117      */
+    const double *z;                 /* host, nz, strictly ascending                             */
+    const heat_layer *layers;        /* host, nlayers                                            */
+    const uint8_t *seg_layer;        /* host, batch*(nr-1): layer of radial segment (i,i+1).
+                                        Node i is an interface node (rows (18)-(20) P:L176-192)
+                                        iff its two segments differ; two interface nodes may
+                                        not be adjacent                                          */
+    heat_bc r_in, r_out, z_lo, z_hi; /* paper: N0,N0,N0,D(T0); BASELINE configs: N0,N0,D,D       */
+    double T0;                       /* uniform initial temperature (5) P:L86 (if !T_init)       */
+    const double *T_init;            /* optional [batch][nz][nr]; host unless T_init_is_device   */
+    double dt;                       /* tau > 0                                                  */
+    const double *Q0;                /* host, batch: source amplitude; NULL = no source          */
+    int64_t steps_per_period;        /* t_prd / tau (4) P:L79; 0 = no source                     */
+    int64_t steps_on;                /* t_src / tau; nu = 1 while (step in period) < steps_on    */
+    int32_t transient_substeps;      /* (22) P:L212-217: the first tau of each period is taken as
+                                        this many sub-steps of tau/substeps with
+                                        p^2 = 1 - exp(-q/transient_k); paper: 100; 0 = Heaviside */
+    int32_t face_mode;               /* lambda at a half node P:L127: 0 = lambda(mean T),
+                                        1 = mean of lambda(T_a), lambda(T_b) (G3)      */
+    double transient_k;              /* paper: 7                                                 */
+    int32_t nprobes;                 /* <= HEAT_MAX_PROBES                                       */
+    int32_t probe_every;             /* record after every probe_every-th step (>= 1 if nprobes) */
+    const int32_t *probe_ij;         /* host, nprobes*(i,j)                                      */
+    int32_t T_init_is_device;
+    int32_t reserved;
+    double T_lo, T_hi;               /* declared temperature range: every lambda_m, c_Vm must be
+                                        strictly positive on it (HEAT_ERANGE otherwise; the
+                                        paper's printed graphite c_V row is not, G11).
+                                        T_hi <= T_lo disables the check                          */
+} heat_desc;
+
+/* Bytes of device workspace heat_create needs for this descriptor (0 if it is malformed). */
+size_t heat_workspace_bytes(const heat_desc *d);
+
+/* Right-hand side of the stability bound (21) P:L194-196,
+ *   tau <= (min_j eta_j^2 / 2) * min_{m,T} rho_m c_Vm(T) / lambda_m(T),
+ * the second minimum over the layers and T in [T_lo, T_hi] (1025 equidistant samples).
+ * Host-only; does not touch the device. */
+heat_status heat_stable_dt(const heat_desc *d, double T_lo, double T_hi, double *dt_limit);
+
+/* Validate the descriptor, derive the per-node row tables, upload them into `workspace`
+ * and initialise both field levels (initial condition (5), Dirichlet sides held from t=0).
+ *   field_a, field_b : device, batch*nz*nr doubles each, 16-byte aligned, caller-owned
+ *   workspace        : device, >= heat_workspace_bytes(d), 256-byte aligned, caller-owned
+ *   probe_buf        : device, probe_cap doubles (may be NULL if nprobes == 0); records of
+ *                      batch*nprobes doubles are appended until it is full, then dropped
+ *   cuda_stream      : cudaStream_t used for the uploads; the call synchronises it
+ * On failure *out is NULL and heat_last_error(NULL) describes why. */
+heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *workspace,
+                        size_t workspace_bytes, void *probe_buf, size_t probe_cap,
+                        void *cuda_stream, heat_ctx **out);
+
+/* Enqueue n solver steps on cuda_stream (asynchronous).  A transient sub-step counts as one
+ * step.  The schedule (tau_k, nu_k p_k^2) is derived from integer step counters only. */
+heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream);
+
+/* Copy the current level of batch member b ([nz][nr], r fastest) to dst.  Asynchronous if
+ * dst is a device pointer; synchronises the stream if dst is host memory. */
+heat_status heat_get_field(heat_ctx *c, int32_t b, double *dst, int32_t dst_is_device,
+                           void *cuda_stream);
+
+/* Overwrite the current level of batch member b (both levels' z-boundary lines included)
+ * and set the solver step counter (checkpoint / resume, snapshot-seeded parity windows). */
+heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t src_is_device,
+                           int64_t step_index, void *cuda_stream);
+
+/* Drain the probe trace: synchronise cuda_stream, copy up to max doubles (whole records of
+ * batch*nprobes doubles, order [record][batch][probe]) to dst_host, and rewind the device
+ * buffer.  *n_written = doubles copied; *n_dropped (optional) = records lost to overflow. */
+heat_status heat_probe(heat_ctx *c, double *dst_host, int64_t max, int64_t *n_written,
+                       int64_t *n_dropped, void *cuda_stream);
+
+/* (tau_k, amplitude_k) of solver step s under this context's schedule (host-only). */
+heat_status heat_schedule(const heat_ctx *c, int64_t s, double *tau, double *amp);
+
+/* Solver steps enqueued so far. */
+int64_t heat_step_index(const heat_ctx *c);
+
+/* Number of kernels this context has launched since creation (bench accounting). */
+int64_t heat_launch_count(const heat_ctx *c);
+
+/* Name of the kernel variant heat_step launches for this context, e.g. "line<M=16,G=512>". */
+const char *heat_kernel_name(const heat_ctx *c);
+
+/* Message of the last failure on this context (c != NULL) or of the last failed
+ * heat_create / heat_stable_dt on the calling thread (c == NULL).  Never NULL. */
+const char *heat_last_error(const heat_ctx *c);
+
+void heat_destroy(heat_ctx *c);
+
+/* Measured-peak helper for the roofline: runs a dependent-chain-free DFMA loop on every SM
+ * and returns the achieved fp64 FMA rate in TFLOP/s (2 flops per FMA); iters per thread.
+ * Not part of the method; allocates and frees its own small scratch buffer. */
+heat_status heat_fp64_peak(int64_t iters, void *cuda_stream, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEAT_B200_H */

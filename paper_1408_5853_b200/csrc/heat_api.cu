@@ -1,0 +1,592 @@
+// heat_api.cu -- the C-ABI of include/heat.h: validation, per-node row tables, the step
+// schedule and kernel launches.  No CPU implementation of the time step lives here: every
+// step of the method runs in the kernels of heat_line_kernel.cuh.
+#include "../../include/heat.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "heat_line_kernel.cuh"
+
+using namespace heat;
+
+namespace {
+
+thread_local std::string g_last_error = "";
+
+void set_err(std::string *dst, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_last_error = buf;
+    if (dst) *dst = buf;
+}
+
+// ---------------------------------------------------------------- kernel variants
+typedef void (*kernel_fn)(const KParams);
+struct Variant {
+    int M, G, tpb, lpb;
+    kernel_fn fn;
+    const char *name;
+    size_t smem_fixed; // bytes without the layer table
+};
+
+#define HEAT_VARIANT(M_, G_)                                                                      \
+    {                                                                                             \
+        M_, G_, LineCfg<M_, G_>::TPB, LineCfg<M_, G_>::LPB, heat_line_kernel<M_, G_>,             \
+            "line<M=" #M_ ",G=" #G_ ">", LineCfg<M_, G_>::smem_bytes(0)                           \
+    }
+const Variant k_variants[] = {
+    HEAT_VARIANT(4, 8),    HEAT_VARIANT(4, 16),  HEAT_VARIANT(4, 32),   HEAT_VARIANT(8, 32),
+    HEAT_VARIANT(16, 32),  HEAT_VARIANT(8, 64),  HEAT_VARIANT(16, 64),  HEAT_VARIANT(8, 128),
+    HEAT_VARIANT(16, 128), HEAT_VARIANT(8, 256), HEAT_VARIANT(16, 256), HEAT_VARIANT(8, 512),
+    HEAT_VARIANT(16, 512), HEAT_VARIANT(8, 1024),
+};
+constexpr int k_nvariants = (int)(sizeof(k_variants) / sizeof(k_variants[0]));
+
+// Default choice: the largest M (fewest reduced rows per cell) whose group covers the line.
+// HEAT_VARIANT="M,G" in the environment overrides it (tuning / tests of every variant).
+const Variant *pick_variant(int nr)
+{
+    if (const char *e = getenv("HEAT_VARIANT")) {
+        int M = 0, G = 0;
+        if (sscanf(e, "%d,%d", &M, &G) == 2)
+            for (int v = 0; v < k_nvariants; ++v)
+                if (k_variants[v].M == M && k_variants[v].G == G && M * G >= nr) return &k_variants[v];
+    }
+    static const int order[][2] = {{4, 8},   {4, 16},  {4, 32},   {8, 32},   {16, 32}, {16, 64},
+                                   {16, 128}, {16, 256}, {16, 512}, {8, 1024}};
+    for (auto &o : order)
+        if (o[0] * o[1] >= nr)
+            for (int v = 0; v < k_nvariants; ++v)
+                if (k_variants[v].M == o[0] && k_variants[v].G == o[1]) return &k_variants[v];
+    return nullptr;
+}
+
+// ---------------------------------------------------------------- host-side law helpers
+double host_law(const heat_law &L, double T)
+{
+    switch (L.kind) {
+    case HEAT_LAW_CONST: return L.c[0];
+    case HEAT_LAW_POWER: return L.c[0] * std::pow(T / L.T_ref, L.c[1]);
+    default: return L.c[0] + T * (L.c[1] + T * (L.c[2] + T * (L.c[3] + T * L.c[4])));
+    }
+}
+
+DLaw fold_law(const heat_law &L, double scale)
+{
+    DLaw d;
+    memset(&d, 0, sizeof d);
+    if (L.kind == HEAT_LAW_CONST || (L.kind == HEAT_LAW_POWER && L.c[1] == 0.0)) {
+        d.kind = LK_CONST;
+        d.ck = d.ckh = scale * L.c[0];
+    } else if (L.kind == HEAT_LAW_POWER) {
+        const long double p = L.c[1];
+        const long double ck = (long double)scale * (long double)L.c[0] / powl((long double)L.T_ref, p);
+        d.ck = (double)ck;
+        d.ckh = (double)(ck * powl(0.5L, p));
+        d.p = L.c[1];
+        if (L.c[1] == 1.0) d.kind = LK_POW1;
+        else if (L.c[1] == 2.0) d.kind = LK_POW2;
+        else if (L.c[1] == 3.0) d.kind = LK_POW3;
+        else if (L.c[1] == 1.5) d.kind = LK_POW1_5;
+        else if (L.c[1] == 0.5) d.kind = LK_POW0_5;
+        else if (L.c[1] == -0.5) d.kind = LK_POWM0_5;
+        else d.kind = LK_POWG;
+    } else {
+        d.kind = LK_POLY;
+        for (int k = 0; k < 5; ++k) d.c[k] = scale * L.c[k];
+    }
+    return d;
+}
+
+bool law_ok(const heat_law &L)
+{
+    if (L.kind != HEAT_LAW_CONST && L.kind != HEAT_LAW_POWER && L.kind != HEAT_LAW_POLY) return false;
+    if (L.kind == HEAT_LAW_POWER && !(L.T_ref > 0.0)) return false;
+    for (int k = 0; k < 5; ++k)
+        if (!std::isfinite(L.c[k])) return false;
+    return true;
+}
+
+bool bc_ok(const heat_bc &b)
+{
+    return (b.kind == HEAT_BC_NEUMANN0 || b.kind == HEAT_BC_DIRICHLET) && std::isfinite(b.value);
+}
+
+constexpr int k_range_samples = 1025;
+
+// ---------------------------------------------------------------- workspace layout
+struct Layout {
+    int nrp;
+    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, total;
+};
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+Layout make_layout(const heat_desc *d, const Variant *v)
+{
+    Layout L;
+    L.nrp = v->M * v->G;
+    size_t o = 0;
+    L.off_ga = o;     o = align_up(o + sizeof(double) * (size_t)d->batch * L.nrp, 256);
+    L.off_gc = o;     o = align_up(o + sizeof(double) * (size_t)d->batch * L.nrp, 256);
+    L.off_info = o;   o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * L.nrp, 256);
+    L.off_ezm = o;    o = align_up(o + sizeof(double) * (size_t)d->nz, 256);
+    L.off_ezp = o;    o = align_up(o + sizeof(double) * (size_t)d->nz, 256);
+    L.off_layers = o; o = align_up(o + sizeof(DLayer) * (size_t)HEAT_MAX_LAYERS, 256);
+    L.off_q0 = o;     o = align_up(o + sizeof(double) * (size_t)d->batch, 256);
+    L.off_probes = o; o = align_up(o + sizeof(ProbeSrc) * (size_t)HEAT_MAX_PROBES, 256);
+    L.total = o;
+    return L;
+}
+
+// Descriptor checks that need no device.  Returns HEAT_OK or the failing status.
+heat_status validate(const heat_desc *d, std::string *err)
+{
+    if (!d) { set_err(err, "descriptor is NULL"); return HEAT_EINVAL; }
+    if (d->nr < 3 || d->nz < 3 || d->batch < 1) { set_err(err, "need nr,nz >= 3 and batch >= 1 (got %d,%d,%d)", d->nr, d->nz, d->batch); return HEAT_EINVAL; }
+    if (d->nr > HEAT_MAX_NR) { set_err(err, "nr = %d exceeds HEAT_MAX_NR = %d", d->nr, HEAT_MAX_NR); return HEAT_EINVAL; }
+    if (d->nlayers < 1 || d->nlayers > HEAT_MAX_LAYERS) { set_err(err, "nlayers = %d outside 1..%d", d->nlayers, HEAT_MAX_LAYERS); return HEAT_EINVAL; }
+    if (!d->r || !d->z || !d->layers || !d->seg_layer) { set_err(err, "r, z, layers and seg_layer must be non-NULL"); return HEAT_EINVAL; }
+    if ((double)d->batch * d->nz * d->nr > 4.0e9) { set_err(err, "batch*nz*nr too large"); return HEAT_EINVAL; }
+    if ((long long)d->batch * (d->nz - 2) > 2000000000LL) { set_err(err, "too many lines"); return HEAT_EINVAL; }
+    if (!(d->dt > 0.0) || !std::isfinite(d->dt)) { set_err(err, "dt must be positive and finite"); return HEAT_EINVAL; }
+    if (!(d->r[0] >= 0.0)) { set_err(err, "r[0] must be >= 0"); return HEAT_EINVAL; }
+    for (int i = 1; i < d->nr; ++i)
+        if (!(d->r[i] > d->r[i - 1])) { set_err(err, "r must be strictly ascending (node %d)", i); return HEAT_EINVAL; }
+    for (int j = 1; j < d->nz; ++j)
+        if (!(d->z[j] > d->z[j - 1])) { set_err(err, "z must be strictly ascending (node %d)", j); return HEAT_EINVAL; }
+    if (!bc_ok(d->r_in) || !bc_ok(d->r_out) || !bc_ok(d->z_lo) || !bc_ok(d->z_hi)) { set_err(err, "bad boundary condition"); return HEAT_EINVAL; }
+    for (int m = 0; m < d->nlayers; ++m) {
+        const heat_layer &L = d->layers[m];
+        if (!law_ok(L.k) || !law_ok(L.cp) || !law_ok(L.src_shape) || !(L.rho > 0.0) || !std::isfinite(L.rho)) {
+            set_err(err, "layer %d: malformed law or non-positive density", m);
+            return HEAT_EINVAL;
+        }
+    }
+    for (int b = 0; b < d->batch; ++b) {
+        const uint8_t *seg = d->seg_layer + (size_t)b * (d->nr - 1);
+        for (int i = 0; i < d->nr - 1; ++i)
+            if (seg[i] >= d->nlayers) { set_err(err, "seg_layer[%d][%d] = %d >= nlayers", b, i, (int)seg[i]); return HEAT_EINVAL; }
+        for (int i = 1; i < d->nr - 2; ++i)
+            if (seg[i - 1] != seg[i] && seg[i] != seg[i + 1]) { set_err(err, "batch %d: interface nodes %d and %d are adjacent", b, i, i + 1); return HEAT_EINVAL; }
+    }
+    if (d->steps_per_period < 0 || d->steps_on < 0 || d->steps_on > d->steps_per_period) { set_err(err, "need 0 <= steps_on <= steps_per_period"); return HEAT_EINVAL; }
+    if (d->transient_substeps < 0 || d->transient_substeps > 1000000) { set_err(err, "transient_substeps out of range"); return HEAT_EINVAL; }
+    if (d->transient_substeps > 0 && !(d->transient_k > 0.0)) { set_err(err, "transient_k must be positive"); return HEAT_EINVAL; }
+    if (d->face_mode != 0 && d->face_mode != 1) { set_err(err, "face_mode must be 0 or 1"); return HEAT_EINVAL; }
+    if (d->nprobes < 0 || d->nprobes > HEAT_MAX_PROBES) { set_err(err, "nprobes outside 0..%d", HEAT_MAX_PROBES); return HEAT_EINVAL; }
+    if (d->nprobes > 0) {
+        if (d->probe_every < 1 || !d->probe_ij) { set_err(err, "probes need probe_every >= 1 and probe_ij"); return HEAT_EINVAL; }
+        for (int q = 0; q < d->nprobes; ++q) {
+            const int i = d->probe_ij[2 * q], j = d->probe_ij[2 * q + 1];
+            if (i < 0 || i >= d->nr || j < 0 || j >= d->nz) { set_err(err, "probe %d = (%d,%d) outside the grid", q, i, j); return HEAT_EINVAL; }
+        }
+    }
+    // strictly positive laws on the declared range (the paper's own graphite c_V row fails, G11)
+    if (d->T_hi > d->T_lo) {
+        for (int m = 0; m < d->nlayers; ++m)
+            for (int s = 0; s < k_range_samples; ++s) {
+                const double T = d->T_lo + (d->T_hi - d->T_lo) * (double)s / (double)(k_range_samples - 1);
+                const double k = host_law(d->layers[m].k, T), c = host_law(d->layers[m].cp, T);
+                if (!(k > 0.0) || !(c > 0.0) || !std::isfinite(k) || !std::isfinite(c)) {
+                    set_err(err, "layer %d: %s(%g K) = %g is not strictly positive on [%g, %g]", m,
+                            !(k > 0.0) ? "lambda" : "c_V", T, !(k > 0.0) ? k : c, d->T_lo, d->T_hi);
+                    return HEAT_ERANGE;
+                }
+            }
+    }
+    return HEAT_OK;
+}
+
+} // namespace
+
+// ---------------------------------------------------------------- context
+struct heat_ctx {
+    int nr, nz, batch, nlayers, nprobes, probe_every, face_mode;
+    heat_bc r_in, r_out, z_lo, z_hi;
+    double dt;
+    int64_t P, S;
+    int nsub;
+    std::vector<double> amp_sub; // 1 - exp(-q/k), q = 0..nsub-1, (22) P:L212 (reading G8)
+    const Variant *var;
+    Layout lay;
+    char *ws;
+    double *cur, *nxt; // current / next level
+    double *probe_buf;
+    size_t probe_cap;
+    int64_t rec_enqueued, rec_dropped;
+    int64_t step;
+    int64_t launches;
+    int grid;
+    size_t smem;
+    std::string err;
+    KParams kp;
+};
+
+#define CUDA_TRY(ctx_err, call)                                                                   \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) {                                                                  \
+            set_err(ctx_err, "%s failed: %s", #call, cudaGetErrorString(e_));                     \
+            return HEAT_ECUDA;                                                                    \
+        }                                                                                         \
+    } while (0)
+
+extern "C" {
+
+size_t heat_workspace_bytes(const heat_desc *d)
+{
+    if (validate(d, nullptr) != HEAT_OK) return 0;
+    const Variant *v = pick_variant(d->nr);
+    if (!v) return 0;
+    return make_layout(d, v).total;
+}
+
+heat_status heat_stable_dt(const heat_desc *d, double T_lo, double T_hi, double *dt_limit)
+{
+    if (!d || !dt_limit || !d->z || !d->layers || d->nz < 2 || d->nlayers < 1) { set_err(nullptr, "heat_stable_dt: bad arguments"); return HEAT_EINVAL; }
+    if (!(T_hi >= T_lo)) { set_err(nullptr, "heat_stable_dt: need T_hi >= T_lo"); return HEAT_EINVAL; }
+    // (21) P:L194-196
+    double eta2 = INFINITY, ratio = INFINITY;
+    for (int j = 1; j < d->nz; ++j) {
+        const double e = d->z[j] - d->z[j - 1];
+        eta2 = std::min(eta2, e * e);
+    }
+    for (int m = 0; m < d->nlayers; ++m)
+        for (int s = 0; s < k_range_samples; ++s) {
+            const double T = T_lo + (T_hi - T_lo) * (double)s / (double)(k_range_samples - 1);
+            const double q = std::fabs(d->layers[m].rho * host_law(d->layers[m].cp, T) / host_law(d->layers[m].k, T));
+            ratio = std::min(ratio, q);
+        }
+    *dt_limit = eta2 / 2.0 * ratio;
+    return HEAT_OK;
+}
+
+heat_status heat_schedule(const heat_ctx *c, int64_t s, double *tau, double *amp)
+{
+    if (!c || !tau || !amp || s < 0) return HEAT_EINVAL;
+    // (4) P:L79 and (22) + procedure P:L212-217; integer counters only (G18); the source is
+    // sampled at the start of the step (G9).
+    if (c->P <= 0 || c->S <= 0) { *tau = c->dt; *amp = 0.0; return HEAT_OK; }
+    if (c->nsub > 0) {
+        const int64_t len = (int64_t)c->nsub + c->P - 1; // solver steps per period
+        const int64_t q = s % len;
+        if (q < c->nsub) {
+            *tau = c->dt / (double)c->nsub;
+            *amp = c->amp_sub[(size_t)q];
+        } else {
+            const int64_t g = q - c->nsub + 1; // 1..P-1: index of the tau-step inside the period
+            *tau = c->dt;
+            *amp = (g < c->S) ? 1.0 : 0.0;
+        }
+    } else {
+        *tau = c->dt;
+        *amp = ((s % c->P) < c->S) ? 1.0 : 0.0;
+    }
+    return HEAT_OK;
+}
+
+heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *workspace,
+                        size_t workspace_bytes, void *probe_buf, size_t probe_cap,
+                        void *cuda_stream, heat_ctx **out)
+{
+    if (out) *out = nullptr;
+    if (!out) { set_err(nullptr, "out is NULL"); return HEAT_EINVAL; }
+    heat_status vs = validate(d, nullptr);
+    if (vs != HEAT_OK) return vs;
+    if (!field_a || !field_b || !workspace || field_a == field_b) { set_err(nullptr, "field_a, field_b (distinct) and workspace must be non-NULL device pointers"); return HEAT_EINVAL; }
+    if (((uintptr_t)field_a | (uintptr_t)field_b) & 15u) { set_err(nullptr, "field buffers must be 16-byte aligned"); return HEAT_EINVAL; }
+    if ((uintptr_t)workspace & 255u) { set_err(nullptr, "workspace must be 256-byte aligned"); return HEAT_EINVAL; }
+    const Variant *v = pick_variant(d->nr);
+    if (!v) { set_err(nullptr, "no kernel variant covers nr = %d", d->nr); return HEAT_EINVAL; }
+    const Layout L = make_layout(d, v);
+    if (workspace_bytes < L.total) { set_err(nullptr, "workspace has %zu bytes, need %zu", workspace_bytes, L.total); return HEAT_ENOMEM; }
+    const size_t rec = (size_t)d->batch * (size_t)d->nprobes;
+    if (d->nprobes > 0 && (!probe_buf || probe_cap < rec)) { set_err(nullptr, "probe buffer must hold at least one record (%zu doubles)", rec); return HEAT_ENOMEM; }
+
+    // ---- device check: this library is sm_100-only, no fallback
+    int dev = 0;
+    cudaDeviceProp prop;
+    CUDA_TRY(nullptr, cudaGetDevice(&dev));
+    CUDA_TRY(nullptr, cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) { set_err(nullptr, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); return HEAT_ECUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    heat_ctx *c = new (std::nothrow) heat_ctx();
+    if (!c) { set_err(nullptr, "out of host memory"); return HEAT_ENOMEM; }
+    c->nr = d->nr; c->nz = d->nz; c->batch = d->batch; c->nlayers = d->nlayers;
+    c->nprobes = d->nprobes; c->probe_every = d->nprobes > 0 ? d->probe_every : 1; c->face_mode = d->face_mode;
+    c->r_in = d->r_in; c->r_out = d->r_out; c->z_lo = d->z_lo; c->z_hi = d->z_hi;
+    c->dt = d->dt; c->P = d->steps_per_period; c->S = d->steps_on; c->nsub = d->transient_substeps;
+    if (!d->Q0) { c->P = 0; c->S = 0; }
+    c->amp_sub.resize((size_t)c->nsub);
+    for (int q = 0; q < c->nsub; ++q) c->amp_sub[(size_t)q] = 1.0 - std::exp(-(double)q / d->transient_k);
+    c->var = v; c->lay = L; c->ws = (char *)workspace;
+    c->cur = (double *)field_a; c->nxt = (double *)field_b;
+    c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
+    c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0;
+
+    // ---- per-node row tables (host), SURVEY 8(a) a4
+    const int nr = d->nr, nz = d->nz, N = nr - 1, nrp = L.nrp;
+    std::vector<double> ga((size_t)d->batch * nrp, 0.0), gc((size_t)d->batch * nrp, 0.0);
+    std::vector<uint32_t> info((size_t)d->batch * nrp, NK_FIXED | (2u << 2));
+    const double *r = d->r;
+    for (int b = 0; b < d->batch; ++b) {
+        const uint8_t *seg = d->seg_layer + (size_t)b * (nr - 1);
+        double *gab = ga.data() + (size_t)b * nrp, *gcb = gc.data() + (size_t)b * nrp;
+        uint32_t *ib = info.data() + (size_t)b * nrp;
+        // (15) P:L158-161:  T^_0 - T^_1 = 0,  T^_N - T^_{N-1} = 0; or Dirichlet rows
+        ib[0] = NK_FIXED | (0u << 2);
+        gab[0] = 0.0; gcb[0] = (d->r_in.kind == HEAT_BC_NEUMANN0) ? -1.0 : 0.0;
+        ib[N] = NK_FIXED | (1u << 2);
+        gab[N] = (d->r_out.kind == HEAT_BC_NEUMANN0) ? -1.0 : 0.0; gcb[N] = 0.0;
+        for (int i = 1; i < N; ++i) {
+            const long double h_i = (long double)r[i] - (long double)r[i - 1];
+            const long double h_ip = (long double)r[i + 1] - (long double)r[i];
+            const uint32_t m = seg[i - 1], m1 = seg[i];
+            if (m == m1) {
+                // (13) P:L140-143 with the prefactor 1/(r_i hbar_i) (reading G1)
+                const long double hbar = (h_i + h_ip) / 2;
+                const long double r_mh = ((long double)r[i] + (long double)r[i - 1]) / 2;
+                const long double r_ph = ((long double)r[i] + (long double)r[i + 1]) / 2;
+                gab[i] = (double)(r_mh / ((long double)r[i] * hbar * h_i));
+                gcb[i] = (double)(r_ph / ((long double)r[i] * hbar * h_ip));
+                ib[i] = NK_REG | (m << 8) | (m << 16);
+            } else {
+                // (18) P:L178-181 times h_i h_{i+1}: -lam_m h_{i+1} x_{i-1} + (...) x_i - lam_{m+1} h_i x_{i+1} = 0
+                gab[i] = (double)h_ip;
+                gcb[i] = (double)h_i;
+                ib[i] = NK_IFACE | (m << 8) | (m1 << 16);
+            }
+        }
+    }
+    std::vector<double> ezm((size_t)nz, 0.0), ezp((size_t)nz, 0.0);
+    for (int j = 1; j < nz - 1; ++j) {
+        const long double e_j = (long double)d->z[j] - (long double)d->z[j - 1];
+        const long double e_jp = (long double)d->z[j + 1] - (long double)d->z[j];
+        const long double ebar = (e_j + e_jp) / 2; // reading G2
+        ezm[(size_t)j] = (double)(1 / (ebar * e_j));
+        ezp[(size_t)j] = (double)(1 / (ebar * e_jp));
+    }
+    std::vector<DLayer> lay((size_t)HEAT_MAX_LAYERS);
+    memset(lay.data(), 0, sizeof(DLayer) * lay.size());
+    for (int m = 0; m < d->nlayers; ++m) {
+        lay[(size_t)m].k = fold_law(d->layers[m].k, 1.0);
+        lay[(size_t)m].rc = fold_law(d->layers[m].cp, d->layers[m].rho);
+        lay[(size_t)m].src = fold_law(d->layers[m].src_shape, 1.0);
+        lay[(size_t)m].heater = d->layers[m].is_heater ? 1 : 0;
+    }
+    std::vector<double> q0((size_t)d->batch, 0.0);
+    if (d->Q0) memcpy(q0.data(), d->Q0, sizeof(double) * (size_t)d->batch);
+    std::vector<ProbeSrc> pr((size_t)HEAT_MAX_PROBES);
+    memset(pr.data(), 0, sizeof(ProbeSrc) * pr.size());
+    for (int q = 0; q < d->nprobes; ++q) {
+        ProbeSrc &s = pr[(size_t)q];
+        s.i = d->probe_ij[2 * q];
+        s.j_store = d->probe_ij[2 * q + 1];
+        s.j_src = s.j_store;
+        s.is_static = 0;
+        if (s.j_store == 0) {
+            if (d->z_lo.kind == HEAT_BC_NEUMANN0) s.j_src = 1; else s.is_static = 1;
+        } else if (s.j_store == nz - 1) {
+            if (d->z_hi.kind == HEAT_BC_NEUMANN0) s.j_src = nz - 2; else s.is_static = 1;
+        }
+    }
+
+    auto fail = [&](heat_status s) { delete c; return s; };
+#define UP(off, vec, type)                                                                        \
+    do {                                                                                          \
+        cudaError_t e_ = cudaMemcpyAsync(c->ws + (off), (vec).data(), sizeof(type) * (vec).size(), \
+                                         cudaMemcpyHostToDevice, st);                             \
+        if (e_ != cudaSuccess) { set_err(nullptr, "upload failed: %s", cudaGetErrorString(e_)); return fail(HEAT_ECUDA); } \
+    } while (0)
+    UP(L.off_ga, ga, double);
+    UP(L.off_gc, gc, double);
+    UP(L.off_info, info, uint32_t);
+    UP(L.off_ezm, ezm, double);
+    UP(L.off_ezp, ezp, double);
+    UP(L.off_layers, lay, DLayer);
+    UP(L.off_q0, q0, double);
+    UP(L.off_probes, pr, ProbeSrc);
+#undef UP
+
+    // ---- initial condition (5) P:L86; Dirichlet sides hold their value from t = 0 (6);
+    //      r sides first, z lines last so that corners belong to the z lines (G17)
+    const size_t cells = (size_t)d->batch * nz * nr;
+    cudaError_t e;
+    if (d->T_init) {
+        e = cudaMemcpyAsync(c->cur, d->T_init, sizeof(double) * cells,
+                            d->T_init_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { set_err(nullptr, "T_init copy failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+    } else {
+        std::vector<double> one((size_t)nz * nr, d->T0);
+        if (d->r_in.kind == HEAT_BC_DIRICHLET) for (int j = 0; j < nz; ++j) one[(size_t)j * nr] = d->r_in.value;
+        if (d->r_out.kind == HEAT_BC_DIRICHLET) for (int j = 0; j < nz; ++j) one[(size_t)j * nr + N] = d->r_out.value;
+        if (d->z_lo.kind == HEAT_BC_DIRICHLET) for (int i = 0; i < nr; ++i) one[(size_t)i] = d->z_lo.value;
+        if (d->z_hi.kind == HEAT_BC_DIRICHLET) for (int i = 0; i < nr; ++i) one[(size_t)(nz - 1) * nr + i] = d->z_hi.value;
+        for (int b = 0; b < d->batch; ++b) {
+            e = cudaMemcpyAsync(c->cur + (size_t)b * nz * nr, one.data(), sizeof(double) * one.size(), cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) { set_err(nullptr, "T0 upload failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        }
+        e = cudaStreamSynchronize(st); // `one` is pageable host memory reused across copies
+        if (e != cudaSuccess) { set_err(nullptr, "stream sync failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+    }
+    e = cudaMemcpyAsync(c->nxt, c->cur, sizeof(double) * cells, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) { set_err(nullptr, "level copy failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+
+    // ---- launch configuration
+    c->smem = v->smem_fixed + sizeof(DLayer) * (size_t)d->nlayers;
+    e = cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+    if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", v->name, c->smem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)v->fn, v->tpb, c->smem);
+    if (e != cudaSuccess || occ < 1) { set_err(nullptr, "%s does not fit on an SM (%s)", v->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+    const long long total_lines = (long long)d->batch * (nz - 2);
+    const long long want = (total_lines + v->lpb - 1) / v->lpb;
+    int occ_cap = occ;
+    if (const char *eo = getenv("HEAT_BLOCKS_PER_SM")) occ_cap = std::max(1, std::min(occ, atoi(eo)));
+    c->grid = (int)std::min<long long>(want, (long long)prop.multiProcessorCount * occ_cap);
+
+    KParams &k = c->kp;
+    memset(&k, 0, sizeof k);
+    k.ga = (const double *)(c->ws + L.off_ga);
+    k.gc = (const double *)(c->ws + L.off_gc);
+    k.info = (const uint32_t *)(c->ws + L.off_info);
+    k.ezm = (const double *)(c->ws + L.off_ezm);
+    k.ezp = (const double *)(c->ws + L.off_ezp);
+    k.layers = (const DLayer *)(c->ws + L.off_layers);
+    k.Q0 = (const double *)(c->ws + L.off_q0);
+    k.probes = (const ProbeSrc *)(c->ws + L.off_probes);
+    k.fixF[0] = (d->r_in.kind == HEAT_BC_DIRICHLET) ? d->r_in.value : 0.0;
+    k.fixF[1] = (d->r_out.kind == HEAT_BC_DIRICHLET) ? d->r_out.value : 0.0;
+    k.fixF[2] = 0.0; k.fixF[3] = 0.0;
+    k.nr = nr; k.nz = nz; k.batch = d->batch; k.nrp = nrp; k.nlayers = d->nlayers; k.nprobes = d->nprobes;
+    k.face_mode = d->face_mode;
+    k.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
+    k.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
+    k.total_lines = (int)total_lines;
+
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { set_err(nullptr, "stream sync failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+    *out = c;
+    return HEAT_OK;
+}
+
+heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
+{
+    if (!c || n < 0) return HEAT_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t rec = (size_t)c->batch * (size_t)c->nprobes;
+    for (int64_t s = 0; s < n; ++s) {
+        double tau, amp;
+        heat_schedule(c, c->step, &tau, &amp);
+        KParams &k = c->kp;
+        k.Told = c->cur;
+        k.Tnew = c->nxt;
+        k.inv_tau = 1.0 / tau;
+        k.amp = amp;
+        k.probe_out = nullptr;
+        if (c->nprobes > 0 && (c->step + 1) % c->probe_every == 0) {
+            if (((size_t)c->rec_enqueued + 1) * rec <= c->probe_cap) {
+                k.probe_out = c->probe_buf + (size_t)c->rec_enqueued * rec;
+                c->rec_enqueued += 1;
+            } else {
+                c->rec_dropped += 1;
+            }
+        }
+        c->var->fn<<<c->grid, c->var->tpb, c->smem, st>>>(k);
+        c->launches += 1;
+        std::swap(c->cur, c->nxt);
+        c->step += 1;
+    }
+    CUDA_TRY(&c->err, cudaGetLastError());
+    return HEAT_OK;
+}
+
+heat_status heat_get_field(heat_ctx *c, int32_t b, double *dst, int32_t dst_is_device, void *cuda_stream)
+{
+    if (!c || !dst || b < 0 || b >= c->batch) { if (c) set_err(&c->err, "heat_get_field: bad arguments"); return HEAT_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)c->nz * c->nr;
+    CUDA_TRY(&c->err, cudaMemcpyAsync(dst, c->cur + (size_t)b * n, sizeof(double) * n,
+                                      dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (!dst_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
+    return HEAT_OK;
+}
+
+heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t src_is_device,
+                           int64_t step_index, void *cuda_stream)
+{
+    if (!c || !src || b < 0 || b >= c->batch || step_index < 0) { if (c) set_err(&c->err, "heat_set_field: bad arguments"); return HEAT_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)c->nz * c->nr;
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    // both levels: the Dirichlet z lines are never written by a step (G17)
+    CUDA_TRY(&c->err, cudaMemcpyAsync(c->cur + (size_t)b * n, src, sizeof(double) * n, kind, st));
+    CUDA_TRY(&c->err, cudaMemcpyAsync(c->nxt + (size_t)b * n, c->cur + (size_t)b * n, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    if (!src_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
+    c->step = step_index;
+    return HEAT_OK;
+}
+
+heat_status heat_probe(heat_ctx *c, double *dst_host, int64_t max, int64_t *n_written,
+                       int64_t *n_dropped, void *cuda_stream)
+{
+    if (!c || max < 0 || (max > 0 && !dst_host)) { if (c) set_err(&c->err, "heat_probe: bad arguments"); return HEAT_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(&c->err, cudaStreamSynchronize(st));
+    const int64_t rec = (int64_t)c->batch * c->nprobes;
+    int64_t nrec = rec > 0 ? std::min<int64_t>(c->rec_enqueued, max / rec) : 0;
+    if (nrec > 0) CUDA_TRY(&c->err, cudaMemcpy(dst_host, c->probe_buf, sizeof(double) * (size_t)(nrec * rec), cudaMemcpyDeviceToHost));
+    if (n_written) *n_written = nrec * rec;
+    if (n_dropped) *n_dropped = c->rec_dropped + (c->rec_enqueued - nrec);
+    c->rec_enqueued = 0;
+    c->rec_dropped = 0;
+    return HEAT_OK;
+}
+
+int64_t heat_step_index(const heat_ctx *c) { return c ? c->step : -1; }
+int64_t heat_launch_count(const heat_ctx *c) { return c ? c->launches : -1; }
+const char *heat_kernel_name(const heat_ctx *c) { return c ? c->var->name : ""; }
+const char *heat_last_error(const heat_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
+void heat_destroy(heat_ctx *c) { delete c; }
+
+heat_status heat_fp64_peak(int64_t iters, void *cuda_stream, double *tflops)
+{
+    if (!tflops || iters < 1) return HEAT_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    CUDA_TRY(nullptr, cudaGetDevice(&dev));
+    CUDA_TRY(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int tpb = 1024, blocks = sms * 2;
+    double *out = nullptr;
+    CUDA_TRY(nullptr, cudaMalloc(&out, sizeof(double) * (size_t)tpb * blocks));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(nullptr, cudaEventCreate(&e0));
+    CUDA_TRY(nullptr, cudaEventCreate(&e1));
+    fp64_peak_kernel<<<blocks, tpb, 0, st>>>(out, iters / 8 + 1, 0.999999, 1e-7); // warm-up
+    CUDA_TRY(nullptr, cudaEventRecord(e0, st));
+    fp64_peak_kernel<<<blocks, tpb, 0, st>>>(out, iters, 0.999999, 1e-7);
+    CUDA_TRY(nullptr, cudaEventRecord(e1, st));
+    CUDA_TRY(nullptr, cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(nullptr, cudaEventElapsedTime(&ms, e0, e1));
+    *tflops = 2.0 * 8.0 * (double)iters * tpb * blocks / (ms * 1e-3) / 1e12;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    return HEAT_OK;
+}
+
+} // extern "C"

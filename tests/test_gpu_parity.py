@@ -1,0 +1,282 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Bar: max |T_gpu - T_oracle| <= 1e-9 K (BASELINE.json north_star);
+integer / schedule work bit-exact.  Protocol per config: SURVEY.md 8(d) / DESIGN.md "Parity".
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1408_5853_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9  # K, BASELINE.json north_star
+
+
+@pytest.fixture(scope="module")
+def bd():
+    from paper_1408_5853_b200 import build as B
+    B.build()
+    from paper_1408_5853_b200 import binding
+    binding.lib()
+    return binding
+
+
+def oracle_cls():
+    from oracle.heat_oracle import Oracle
+    return Oracle
+
+
+def with_dt(bd, s0, safety=None):
+    """tau from the library's own (21); the same spec then drives both sides."""
+    lim = bd.heat_stable_dt(s0)
+    if safety is None:
+        return I.with_dt(s0, lim)
+    s = dict(s0)
+    s["dt"] = safety * lim
+    return s
+
+
+def compare(sim, orc, tol=TOL):
+    err = 0.0
+    for b in range(sim.batch):
+        g, o = sim.field(b), orc.field(b)
+        assert np.all(np.isfinite(g))
+        err = max(err, float(np.max(np.abs(g - o))))
+    assert err <= tol, f"max |dT| = {err:.3e} K"
+    return err
+
+
+# ----------------------------------------------------------------------------- small general cases
+
+BC_SETS = [
+    (I.NEUMANN0, I.NEUMANN0, I.dirichlet(4.2), I.dirichlet(78.0)),   # BASELINE.json configs
+    (I.NEUMANN0, I.NEUMANN0, I.NEUMANN0, I.dirichlet(4.2)),          # the paper's (6) P:L90-95
+    (I.dirichlet(10.0), I.dirichlet(30.0), I.NEUMANN0, I.NEUMANN0),
+    (I.NEUMANN0, I.dirichlet(25.0), I.dirichlet(5.0), I.NEUMANN0),
+]
+
+
+@pytest.mark.parametrize("seed", range(4))
+@pytest.mark.parametrize("bcs", BC_SETS)
+@pytest.mark.parametrize("face_mode", [0, 1])
+def test_random_small_problems(bd, seed, bcs, face_mode):
+    """Non-uniform grids, odd sizes (ragged tails, scalar-load path), mixed law kinds, all BC
+    kinds, source with sub-stepping, probes, batch of 2."""
+    nr, nz = [(13, 11), (37, 9), (64, 20), (131, 7)][seed]
+    s = I.random_spec(seed, nr=nr, nz=nz, nlayers=3, batch=2, bcs=bcs, r0=0.0 if seed % 2 else 3e-4)
+    s["face_mode"] = face_mode
+    s = with_dt(bd, s, 0.7)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s)
+    for n in (1, 2, 17):
+        sim.step(n)
+        orc.step(n)
+        compare(sim, orc)
+    pg, dropped = sim.probes()
+    po = orc.probes()
+    assert dropped == 0 and pg.shape == po.shape
+    assert np.max(np.abs(pg - po)) <= TOL
+    sim.close()
+
+
+VARIANTS = ["4,8", "4,16", "4,32", "8,32", "16,32", "8,64", "16,64", "8,128", "16,128", "8,256", "16,256",
+            "8,512", "16,512", "8,1024"]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_every_kernel_variant(bd, variant, monkeypatch):
+    """Each (M rows per thread, G threads per line) instantiation on a line that fills it
+    only partly (ragged tail inside the last thread, whole idle threads) and on one that fills
+    it exactly."""
+    M, G = (int(x) for x in variant.split(","))
+    monkeypatch.setenv("HEAT_VARIANT", variant)
+    for nr in (M * G, M * G - M - 3):
+        nz = 7 if nr > 2048 else 12
+        s0 = I.config(2, nr=nr, nz=nz)
+        # keep eta = 10 h as in the BASELINE configs (L/R = 10, nr = nz): otherwise the line
+        # systems of a long thin grid are ill-conditioned and rounding, not the kernel, is tested
+        s0["z"] = I.uniform_nodes(10.0 * (nz - 1) * 2e-3 / (nr - 1), nz)
+        s = with_dt(bd, s0)
+        sim, orc = bd.HeatSim(s), oracle_cls()(s)
+        assert sim.kernel_name == f"line<M={M},G={G}>"
+        sim.step(120)
+        orc.step(120)
+        compare(sim, orc)
+        sim.close()
+
+
+def test_schedule_table_is_bit_exact(bd):
+    """(4) P:L79, (22) P:L212-217: the library's (tau_k, amp_k) equals the oracle's, bitwise."""
+    s = I.random_spec(0, source=True)
+    s["steps_per_period"], s["steps_on"], s["transient_substeps"], s["transient_k"] = 12, 3, 100, 7.0
+    s["dt"] = 1e-6
+    sim, orc = bd.HeatSim(s), oracle_cls()(s)
+    for k in range(2 * 111 + 5):
+        assert sim.schedule(k) == orc.schedule(k)
+    s["transient_substeps"] = 0
+    sim2, orc2 = bd.HeatSim(s), oracle_cls()(s)
+    for k in range(30):
+        assert sim2.schedule(k) == orc2.schedule(k)
+
+
+def test_set_get_field_and_step_index(bd):
+    """Checkpoint / resume: heat_get_field -> heat_set_field reproduces the run bitwise."""
+    s = with_dt(bd, I.config(2, nr=96, nz=40))
+    a = bd.HeatSim(s)
+    a.step(150)
+    snap, k = a.field(0), a.step_index
+    a.step(77)
+    ref = a.field(0)
+    b = bd.HeatSim(s)
+    b.set_field(0, snap, k)
+    b.step(77)
+    assert np.array_equal(b.field(0), ref)
+    c = bd.HeatSim(s)
+    c.set_field(0, a._torch.from_numpy(snap).cuda(), k)   # device source
+    c.step(77)
+    assert np.array_equal(c.field_device(0).cpu().numpy(), ref)
+
+
+def test_batch_member_equals_single_run_bitwise(bd):
+    """Cell b of a batch run == the same cell run alone, bitwise on the GPU."""
+    s = with_dt(bd, I.config(3, nr=128, nz=40, batch=5))
+    sim = bd.HeatSim(s)
+    sim.step(140)
+    for b in (0, 3, 4):
+        s1 = dict(s, batch=1, seg_layer=s["seg_layer"][b:b + 1], Q0=s["Q0"][b:b + 1])
+        one = bd.HeatSim(s1)
+        one.step(140)
+        assert np.array_equal(one.field(0), sim.field(b))
+    assert not np.array_equal(sim.field(0), sim.field(1))
+
+
+def test_dirichlet_lines_and_r_boundary_rows(bd):
+    """G17: Dirichlet z lines are never touched; (15): T^_0 = T^_1 bitwise."""
+    s = with_dt(bd, I.config(1, nr=100, nz=30))
+    sim = bd.HeatSim(s)
+    sim.step(33)
+    T = sim.field(0)
+    assert np.all(T[0] == 4.2) and np.all(T[-1] == 78.0)
+    assert np.array_equal(T[1:-1, 0], T[1:-1, 1])
+    assert np.max(np.abs(T[1:-1, -1] - T[1:-1, -2])) < 1e-12
+
+
+def test_probe_buffer_overflow_is_counted(bd):
+    s = with_dt(bd, I.config(2, nr=64, nz=24))
+    sim = bd.HeatSim(s, probe_records=10)
+    sim.step(25)
+    p, dropped = sim.probes()
+    assert p.shape == (10, 1, 1) and dropped == 15
+    sim.step(4)
+    p, dropped = sim.probes()
+    assert p.shape == (4, 1, 1) and dropped == 0
+
+
+# ----------------------------------------------------------------------------- BASELINE.json configs
+
+def test_config0_full_length(bd):
+    """configs[0]: 64x64 constant coefficients, all 1000 steps."""
+    s = with_dt(bd, I.config(0))
+    sim, orc = bd.HeatSim(s), oracle_cls()(s)
+    sim.step(s["steps"])
+    orc.step(s["steps"])
+    compare(sim, orc)
+
+
+def test_config1_full_length(bd):
+    """configs[1]: 512x512 nonlinear 4-layer cell, 2000 steps from the initial condition."""
+    s = with_dt(bd, I.config(1))
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp")
+    for _ in range(4):
+        sim.step(500)
+        orc.step(500)
+        compare(sim, orc)
+
+
+def test_config2_windows(bd):
+    """configs[2]: 2048x2048 with pulse heating.  W1 = steps 0..299 from the initial condition
+    (100 sub-steps + 200 steps); W2 / W3 = snapshot-seeded windows across switch-off and across
+    the next switch-on (the GPU field at the window start seeds the oracle)."""
+    s = with_dt(bd, I.config(2))
+    assert s["steps_per_period"] == 11199033
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp")
+    sim.step(300)
+    orc.step(300)
+    compare(sim, orc)
+    pg, _ = sim.probes()
+    assert np.max(np.abs(pg - orc.probes())) <= TOL
+    nsub, P, S = s["transient_substeps"], s["steps_per_period"], s["steps_on"]
+    off = nsub + S - 1                      # first solver step with amp = 0
+    for start in (off - 20, nsub + P - 1 - 20):
+        snap = sim.field(0)
+        sim.set_field(0, snap, start)
+        orc.set_field(0, snap, start)
+        sim.step(60)
+        orc.step(60)
+        amps = [sim.schedule(start + q)[1] for q in range(60)]
+        assert len(set(amps)) > 1           # the window really crosses a switch
+        compare(sim, orc)
+
+
+@pytest.mark.parametrize("n", [64, 128])
+def test_config2_downscaled_full_length(bd, n):
+    """configs[2] physics on n x n nodes, all 5 periods (5.3e4 steps at 64^2, 2.2e5 at 128^2): drift check,
+    field and probe trace."""
+    s = with_dt(bd, I.config(2, nr=n, nz=n))
+    sim, orc = bd.HeatSim(s, probe_records=s["steps"] + 8), oracle_cls()(s, variant="omp" if n > 64 else "double")
+    sim.step(s["steps"])
+    orc.step(s["steps"])
+    compare(sim, orc)
+    pg, dropped = sim.probes()
+    po = orc.probes()
+    assert dropped == 0 and pg.shape == po.shape == (s["steps"], 1, 1)
+    assert np.max(np.abs(pg - po)) <= TOL
+
+
+def test_config3_batch_sample(bd):
+    """configs[3]: 256 cells of 512x512.  The whole batch runs on the GPU; cells first, last,
+    max Q0 and max heater thickness are checked against single-cell oracle runs: 300 steps from
+    the initial condition, then a snapshot-seeded window across switch-off."""
+    s = with_dt(bd, I.config(3))
+    sim = bd.HeatSim(s)
+    sim.step(300)
+    cells = sorted({0, 255, int(np.argmax(s["Q0"])), int(np.argmax(s["heater_thickness_mm"]))})
+    orcs = {}
+    for b in cells:
+        s1 = dict(s, batch=1, seg_layer=s["seg_layer"][b:b + 1], Q0=s["Q0"][b:b + 1])
+        o = oracle_cls()(s1, variant="omp")
+        o.step(300)
+        assert np.max(np.abs(sim.field(b) - o.field(0))) <= TOL
+        orcs[b] = o
+    start = s["transient_substeps"] + s["steps_on"] - 1 - 15
+    for b in cells:
+        snap = sim.field(b)
+        orcs[b].set_field(0, snap, start)
+    snaps = sim._torch.stack([sim.field_device(b) for b in range(sim.batch)])
+    for b in range(sim.batch):
+        sim.set_field(b, snaps[b].contiguous(), start)
+    sim.step(40)
+    for b in cells:
+        orcs[b].step(40)
+        assert np.max(np.abs(sim.field(b) - orcs[b].field(0))) <= TOL
+
+
+def test_config4_windows(bd):
+    """configs[4]: 8192x8192, the launch configuration bench.py times.  10 steps from the
+    initial condition; then the GPU runs on to step 9990 and a snapshot-seeded window
+    9990 -> 10000 is compared (probe every 100 steps)."""
+    s = with_dt(bd, I.config(4))
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp")
+    sim.step(10)
+    orc.step(10)
+    compare(sim, orc)
+    sim.step(9980)
+    snap = sim.field(0)
+    orc.set_field(0, snap, 9990)
+    sim.step(10)
+    orc.step(10)
+    compare(sim, orc)
+    pg, dropped = sim.probes()
+    assert pg.shape == (100, 1, 1) and dropped == 0
+    assert abs(pg[-1, 0, 0] - orc.field(0)[s["probes"][0][1], s["probes"][0][0]]) <= TOL
