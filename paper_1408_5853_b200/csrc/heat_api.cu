@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "heat_line_kernel.cuh"
+#include "heat_tma_kernel.cuh"
 
 using namespace heat;
 
@@ -72,6 +73,36 @@ const Variant *pick_variant(int nr)
     return nullptr;
 }
 
+// ---------------------------------------------------------------- TMA kernel variants
+typedef void (*tma_kernel_fn)(const TParams);
+struct TmaVariant {
+    int G, CL;
+    tma_kernel_fn fn;
+    const char *name;
+    size_t smem_fixed; // bytes without the layer table
+};
+#define HEAT_TMA_VARIANT(G_, CL_)                                                                 \
+    {                                                                                             \
+        G_, CL_, heat_tma_kernel<G_, CL_>, "tma<G=" #G_ ",CL=" #CL_ ">", TmaCfg<G_, CL_>::smem_bytes(0) \
+    }
+const TmaVariant k_tma_variants[] = {
+    HEAT_TMA_VARIANT(8, 1),   HEAT_TMA_VARIANT(16, 1),  HEAT_TMA_VARIANT(32, 1),  HEAT_TMA_VARIANT(64, 1),
+    HEAT_TMA_VARIANT(128, 1), HEAT_TMA_VARIANT(128, 2), HEAT_TMA_VARIANT(128, 4),
+};
+
+// The TMA kernel covers lines of 16*G*CL nodes exactly (nr = 128 .. 8192, powers of two);
+// every other nr, HEAT_KERNEL=line or HEAT_VARIANT in the environment select the line kernel.
+const TmaVariant *pick_tma_variant(int nr)
+{
+    if (getenv("HEAT_VARIANT")) return nullptr;
+    if (const char *e = getenv("HEAT_KERNEL"))
+        if (strcmp(e, "line") == 0) return nullptr;
+    if (nr % 16 != 0) return nullptr;
+    for (auto &v : k_tma_variants)
+        if (16 * v.G * v.CL == nr) return &v;
+    return nullptr;
+}
+
 // ---------------------------------------------------------------- host-side law helpers
 double host_law(const heat_law &L, double T)
 {
@@ -128,15 +159,15 @@ constexpr int k_range_samples = 1025;
 // ---------------------------------------------------------------- workspace layout
 struct Layout {
     int nrp;
-    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, total;
+    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, total;
 };
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-Layout make_layout(const heat_desc *d, const Variant *v)
+Layout make_layout(const heat_desc *d, const Variant *v, const TmaVariant *tv)
 {
     Layout L;
-    L.nrp = v->M * v->G;
+    L.nrp = tv ? d->nr : v->M * v->G;
     size_t o = 0;
     L.off_ga = o;     o = align_up(o + sizeof(double) * (size_t)d->batch * L.nrp, 256);
     L.off_gc = o;     o = align_up(o + sizeof(double) * (size_t)d->batch * L.nrp, 256);
@@ -146,6 +177,7 @@ Layout make_layout(const heat_desc *d, const Variant *v)
     L.off_layers = o; o = align_up(o + sizeof(DLayer) * (size_t)HEAT_MAX_LAYERS, 256);
     L.off_q0 = o;     o = align_up(o + sizeof(double) * (size_t)d->batch, 256);
     L.off_probes = o; o = align_up(o + sizeof(ProbeSrc) * (size_t)HEAT_MAX_PROBES, 256);
+    L.off_cdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 16 + 1), 256);
     L.total = o;
     return L;
 }
@@ -220,6 +252,10 @@ struct heat_ctx {
     int nsub;
     std::vector<double> amp_sub; // 1 - exp(-q/k), q = 0..nsub-1, (22) P:L212 (reading G8)
     const Variant *var;
+    const TmaVariant *tvar; // non-NULL: heat_step launches the TMA kernel
+    CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
+    double *field_a;
+    TParams tp;
     Layout lay;
     char *ws;
     double *cur, *nxt; // current / next level
@@ -248,9 +284,10 @@ extern "C" {
 size_t heat_workspace_bytes(const heat_desc *d)
 {
     if (validate(d, nullptr) != HEAT_OK) return 0;
-    const Variant *v = pick_variant(d->nr);
-    if (!v) return 0;
-    return make_layout(d, v).total;
+    const TmaVariant *tv = pick_tma_variant(d->nr);
+    const Variant *v = tv ? nullptr : pick_variant(d->nr);
+    if (!v && !tv) return 0;
+    return make_layout(d, v, tv).total;
 }
 
 heat_status heat_stable_dt(const heat_desc *d, double T_lo, double T_hi, double *dt_limit)
@@ -308,9 +345,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (!field_a || !field_b || !workspace || field_a == field_b) { set_err(nullptr, "field_a, field_b (distinct) and workspace must be non-NULL device pointers"); return HEAT_EINVAL; }
     if (((uintptr_t)field_a | (uintptr_t)field_b) & 15u) { set_err(nullptr, "field buffers must be 16-byte aligned"); return HEAT_EINVAL; }
     if ((uintptr_t)workspace & 255u) { set_err(nullptr, "workspace must be 256-byte aligned"); return HEAT_EINVAL; }
-    const Variant *v = pick_variant(d->nr);
-    if (!v) { set_err(nullptr, "no kernel variant covers nr = %d", d->nr); return HEAT_EINVAL; }
-    const Layout L = make_layout(d, v);
+    const TmaVariant *tv = pick_tma_variant(d->nr);
+    const Variant *v = tv ? nullptr : pick_variant(d->nr);
+    if (!v && !tv) { set_err(nullptr, "no kernel variant covers nr = %d", d->nr); return HEAT_EINVAL; }
+    const Layout L = make_layout(d, v, tv);
     if (workspace_bytes < L.total) { set_err(nullptr, "workspace has %zu bytes, need %zu", workspace_bytes, L.total); return HEAT_ENOMEM; }
     const size_t rec = (size_t)d->batch * (size_t)d->nprobes;
     if (d->nprobes > 0 && (!probe_buf || probe_cap < rec)) { set_err(nullptr, "probe buffer must hold at least one record (%zu doubles)", rec); return HEAT_ENOMEM; }
@@ -332,7 +370,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (!d->Q0) { c->P = 0; c->S = 0; }
     c->amp_sub.resize((size_t)c->nsub);
     for (int q = 0; q < c->nsub; ++q) c->amp_sub[(size_t)q] = 1.0 - std::exp(-(double)q / d->transient_k);
-    c->var = v; c->lay = L; c->ws = (char *)workspace;
+    c->var = v; c->tvar = tv; c->lay = L; c->ws = (char *)workspace;
+    c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
     c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
     c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0;
@@ -404,6 +443,52 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         }
     }
 
+    // ---- chunk classes of the TMA kernel: a 16-node chunk runs class-templated code iff all
+    //      its nodes are regular nodes of one layer whose (lambda, rho c) kinds form a fast
+    //      class, the r grid is uniform from r = 0 (the geometric factors of (13) then are
+    //      (i -+ 1/2)/(i h^2), generated on the fly) and lambda sits at the mean temperature
+    std::vector<uint32_t> cdesc((size_t)d->batch * (size_t)(nr / 16 + 1), CC_GENERIC);
+    double g0 = 0.0;
+    if (tv) {
+        const long double h = ((long double)r[N] - (long double)r[0]) / (long double)N;
+        g0 = (double)(1.0L / (h * h));
+        bool uniform = (r[0] == 0.0) && (d->face_mode == 0);
+        if (const char *e = getenv("HEAT_NO_FAST")) uniform = uniform && atoi(e) == 0;
+        for (int b = 0; b < d->batch && uniform; ++b) {
+            const double *gab = ga.data() + (size_t)b * nrp, *gcb = gc.data() + (size_t)b * nrp;
+            const uint32_t *ib = info.data() + (size_t)b * nrp;
+            for (int i = 1; i < N && uniform; ++i) {
+                if ((ib[i] & 3u) != NK_REG) continue;
+                const long double ea = (long double)g0 * ((long double)i - 0.5L) / (long double)i;
+                const long double ec = (long double)g0 * ((long double)i + 0.5L) / (long double)i;
+                if (fabsl((long double)gab[i] - ea) > 1e-11L * ea || fabsl((long double)gcb[i] - ec) > 1e-11L * ec) uniform = false;
+            }
+        }
+        auto class_of = [&](const DLayer &Lm) -> uint32_t {
+            if (Lm.heater && Lm.src.kind != LK_CONST) return CC_GENERIC;
+            const int kk = Lm.k.kind, ck = Lm.rc.kind;
+            if (kk == LK_CONST && ck == LK_CONST) return CC_K0_C0;
+            if (kk == LK_POW1 && ck == LK_POW3) return CC_K1_C3;
+            if (kk == LK_POW2 && ck == LK_POW3) return CC_K2_C3;
+            if (kk == LK_POW1 && ck == LK_POW2) return CC_K1_C2;
+            if (kk == LK_POW1_5 && ck == LK_POW3) return CC_K15_C3;
+            return CC_GENERIC;
+        };
+        const int rpl = nr / 16;
+        for (int b = 0; b < d->batch && uniform; ++b) {
+            const uint32_t *ib = info.data() + (size_t)b * nrp;
+            for (int t = 0; t < rpl; ++t) {
+                bool ok = true;
+                const uint32_t first = ib[16 * t];
+                for (int k = 0; k < 16 && ok; ++k) ok = ((ib[16 * t + k] & 3u) == NK_REG) && (ib[16 * t + k] == first);
+                if (!ok) continue;
+                const uint32_t m = (first >> 8) & 0xffu;
+                const uint32_t cc = class_of(lay[m]);
+                cdesc[(size_t)b * rpl + t] = cc | (m << 8);
+            }
+        }
+    }
+
     auto fail = [&](heat_status s) { delete c; return s; };
 #define UP(off, vec, type)                                                                        \
     do {                                                                                          \
@@ -419,6 +504,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     UP(L.off_layers, lay, DLayer);
     UP(L.off_q0, q0, double);
     UP(L.off_probes, pr, ProbeSrc);
+    UP(L.off_cdesc, cdesc, uint32_t);
 #undef UP
 
     // ---- initial condition (5) P:L86; Dirichlet sides hold their value from t = 0 (6);
@@ -446,17 +532,73 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (e != cudaSuccess) { set_err(nullptr, "level copy failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
 
     // ---- launch configuration
-    c->smem = v->smem_fixed + sizeof(DLayer) * (size_t)d->nlayers;
-    e = cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
-    if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", v->name, c->smem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
-    int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)v->fn, v->tpb, c->smem);
-    if (e != cudaSuccess || occ < 1) { set_err(nullptr, "%s does not fit on an SM (%s)", v->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
     const long long total_lines = (long long)d->batch * (nz - 2);
-    const long long want = (total_lines + v->lpb - 1) / v->lpb;
-    int occ_cap = occ;
-    if (const char *eo = getenv("HEAT_BLOCKS_PER_SM")) occ_cap = std::max(1, std::min(occ, atoi(eo)));
-    c->grid = (int)std::min<long long>(want, (long long)prop.multiProcessorCount * occ_cap);
+    int occ_cap_env = 0;
+    if (const char *eo = getenv("HEAT_BLOCKS_PER_SM")) occ_cap_env = std::max(1, atoi(eo));
+    if (tv) {
+        c->smem = tv->smem_fixed + sizeof(DLayer) * (size_t)d->nlayers;
+        e = cudaFuncSetAttribute((const void *)tv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+        if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", tv->name, c->smem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        const int lpb = 128 / tv->G;
+        const int spm = (nz - 2 + lpb - 1) / lpb; // slabs per batch member
+        const long long total_slabs = (long long)d->batch * spm;
+        int max_clusters = 0;
+        {
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * 8 * tv->CL) / tv->CL * tv->CL, 1, 1);
+            cfg.blockDim = dim3(128, 1, 1);
+            cfg.dynamicSmemBytes = c->smem;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)tv->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            e = cudaOccupancyMaxActiveClusters(&max_clusters, (const void *)tv->fn, &cfg);
+            if (e != cudaSuccess || max_clusters < 1) { set_err(nullptr, "%s does not fit on the device (%s)", tv->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        }
+        if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / tv->CL);
+        const long long nclusters = std::min<long long>(total_slabs, max_clusters);
+        c->grid = (int)nclusters * tv->CL;
+        // tensor maps: each level as [batch*nz*nr/16 rows][16 doubles], SWIZZLE_128B
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || !sym || qres != cudaDriverEntryPointSuccess) { set_err(nullptr, "cuTensorMapEncodeTiled is unavailable (%s)", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        encode_fn encode = (encode_fn)sym;
+        const cuuint64_t gdim[2] = {16, (cuuint64_t)cells / 16};
+        const cuuint64_t gstr[1] = {128};
+        const cuuint32_t estr[2] = {1, 1};
+        double *lev[2] = {c->cur, c->nxt};
+        for (int q = 0; q < 2; ++q) {
+            const cuuint32_t box_ld[2] = {16, 128}, box_st[2] = {16, (cuuint32_t)tv->G};
+            CUresult r1 = encode(&c->tm_ld[q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, lev[q], gdim, gstr, box_ld, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            CUresult r2 = encode(&c->tm_st[q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, lev[q], gdim, gstr, box_st, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) { set_err(nullptr, "cuTensorMapEncodeTiled failed (%d, %d)", (int)r1, (int)r2); return fail(HEAT_ECUDA); }
+        }
+        memset(&c->tp, 0, sizeof c->tp);
+        c->tp.cdesc = (const uint32_t *)(c->ws + L.off_cdesc);
+        c->tp.g0 = g0;
+        c->tp.rpl = nr / 16;
+        c->tp.slabs_per_member = spm;
+        c->tp.total_slabs = (int)total_slabs;
+    } else {
+        c->smem = v->smem_fixed + sizeof(DLayer) * (size_t)d->nlayers;
+        e = cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+        if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", v->name, c->smem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        int occ = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)v->fn, v->tpb, c->smem);
+        if (e != cudaSuccess || occ < 1) { set_err(nullptr, "%s does not fit on an SM (%s)", v->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        const long long want = (total_lines + v->lpb - 1) / v->lpb;
+        const int occ_cap = occ_cap_env > 0 ? std::min(occ, occ_cap_env) : occ;
+        c->grid = (int)std::min<long long>(want, (long long)prop.multiProcessorCount * occ_cap);
+    }
 
     KParams &k = c->kp;
     memset(&k, 0, sizeof k);
@@ -505,7 +647,25 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
                 c->rec_dropped += 1;
             }
         }
-        c->var->fn<<<c->grid, c->var->tpb, c->smem, st>>>(k);
+        if (c->tvar) {
+            const int q = (c->cur == c->field_a) ? 0 : 1;
+            c->tp.tm_ld = c->tm_ld[q];
+            c->tp.tm_st = c->tm_st[1 - q];
+            c->tp.k = k;
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)c->grid, 1, 1);
+            cfg.blockDim = dim3(128, 1, 1);
+            cfg.dynamicSmemBytes = c->smem;
+            cfg.stream = st;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)c->tvar->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->tvar->fn, c->tp));
+        } else {
+            c->var->fn<<<c->grid, c->var->tpb, c->smem, st>>>(k);
+        }
         c->launches += 1;
         std::swap(c->cur, c->nxt);
         c->step += 1;
@@ -558,7 +718,7 @@ heat_status heat_probe(heat_ctx *c, double *dst_host, int64_t max, int64_t *n_wr
 
 int64_t heat_step_index(const heat_ctx *c) { return c ? c->step : -1; }
 int64_t heat_launch_count(const heat_ctx *c) { return c ? c->launches : -1; }
-const char *heat_kernel_name(const heat_ctx *c) { return c ? c->var->name : ""; }
+const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->tvar ? c->tvar->name : c->var->name) : ""; }
 const char *heat_last_error(const heat_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
 void heat_destroy(heat_ctx *c) { delete c; }
 
