@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libheat_b200.so")
 SOURCES = [os.path.join(CSRC, "heat_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("heat_device.cuh", "heat_line_kernel.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh")] + [
     os.path.join(ROOT, "include", "heat.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
