@@ -15,11 +15,22 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libheat_b200.so")
-SOURCES = [os.path.join(CSRC, "heat_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh")] + [
-    os.path.join(ROOT, "include", "heat.h")]
+def _c(*names):
+    return [os.path.join(CSRC, n) for n in names]
+
+
+HEAT_H = os.path.join(ROOT, "include", "heat.h")
+# translation unit -> the files it is built from
+UNITS = {
+    "heat_api.cu": _c("heat_api.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                      "heat_band_params.cuh", "heat_band_variants.h") + [HEAT_H],
+    "heat_band.cu": _c("heat_band.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                       "heat_band_params.cuh", "heat_band_variants.h", "heat_band_kernel.cuh"),
+}
+SOURCES = _c(*UNITS)
+DEPS = sorted({d for deps in UNITS.values() for d in deps})
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
 def nvcc() -> str:
@@ -37,15 +48,31 @@ def up_to_date() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile the library if any source is newer than it; return its path."""
+    """Compile the library if any source is newer than it; return its path.  The translation
+    units are compiled side by side (nvcc -c), then linked into one shared object."""
     if not force and up_to_date():
         return LIB
-    cmd = [nvcc(), *NVCC_FLAGS, "-o", LIB, *SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    log = res.stdout + res.stderr
+    objs = [os.path.splitext(src)[0] + ".o" for src in SOURCES]
+    cmds = []
+    for (unit, deps), src, obj in zip(UNITS.items(), SOURCES, objs):
+        stale = force or not os.path.exists(obj) or any(os.path.getmtime(d) > os.path.getmtime(obj) for d in deps)
+        if stale:
+            cmds.append([nvcc(), *NVCC_FLAGS, "-c", "-o", obj, src])
+    procs = [subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for cmd in cmds]
+    log = ""
+    failed = False
+    for cmd, pr in zip(cmds, procs):
+        out, _ = pr.communicate()
+        log += " ".join(cmd) + "\n" + out
+        failed = failed or pr.returncode != 0
+    if not failed:
+        link = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB, *objs]
+        res = subprocess.run(link, capture_output=True, text=True)
+        log += " ".join(link) + "\n" + res.stdout + res.stderr
+        failed = res.returncode != 0
     with open(os.path.join(HERE, "build.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + log)
-    if res.returncode != 0:
+        f.write(log)
+    if failed:
         raise RuntimeError("nvcc failed:\n" + log[-4000:])
     if verbose:
         print(log)

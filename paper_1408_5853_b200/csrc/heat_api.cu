@@ -14,6 +14,7 @@
 
 #include "heat_line_kernel.cuh"
 #include "heat_tma_kernel.cuh"
+#include "heat_band_variants.h"
 
 using namespace heat;
 
@@ -103,6 +104,7 @@ const TmaVariant *pick_tma_variant(int nr)
     return nullptr;
 }
 
+
 // ---------------------------------------------------------------- host-side law helpers
 double host_law(const heat_law &L, double T)
 {
@@ -154,12 +156,124 @@ bool bc_ok(const heat_bc &b)
     return (b.kind == HEAT_BC_NEUMANN0 || b.kind == HEAT_BC_DIRICHLET) && std::isfinite(b.value);
 }
 
+
+// ---------------------------------------------------------------- band kernel planning (host)
+// Laws of a layer in the polynomial form of heat_band_kernel.cuh; false if a law has no such form.
+bool to_player(const heat_layer &L, PLayer *out, int *degk)
+{
+    PLayer P;
+    memset(&P, 0, sizeof P);
+    *degk = 0;
+    const heat_law &k = L.k;
+    if (k.kind == HEAT_LAW_CONST) {
+        P.K[0] = k.c[0];
+    } else if (k.kind == HEAT_LAW_POWER) {
+        const long double p = k.c[1];
+        const long double ckh = (long double)k.c[0] / powl((long double)k.T_ref, p) * powl(0.5L, p);
+        if (k.c[1] == 0.0) P.K[0] = (double)ckh;
+        else if (k.c[1] == 1.0) { P.K[1] = (double)ckh; *degk = 1; }
+        else if (k.c[1] == 2.0) { P.K[2] = (double)ckh; *degk = 2; }
+        else if (k.c[1] == 3.0) { P.K[3] = (double)ckh; *degk = 3; }
+        else if (k.c[1] == 1.5) { P.K[1] = (double)ckh; P.sqrtk = 1; *degk = 1; }
+        else if (k.c[1] == 0.5) { P.K[0] = (double)ckh; P.sqrtk = 1; }
+        else return false;
+    } else {
+        long double hp = 1.0L;
+        for (int n = 0; n < 5; ++n) {
+            P.K[n] = (double)((long double)k.c[n] * hp);
+            hp *= 0.5L;
+            if (k.c[n] != 0.0) *degk = n;
+        }
+    }
+    const heat_law &c = L.cp;
+    if (c.kind == HEAT_LAW_CONST) {
+        P.C[0] = L.rho * c.c[0];
+    } else if (c.kind == HEAT_LAW_POWER) {
+        const long double q = c.c[1];
+        const long double cq = (long double)L.rho * (long double)c.c[0] / powl((long double)c.T_ref, q);
+        if (c.c[1] == 0.0) P.C[0] = (double)cq;
+        else if (c.c[1] == 1.0) P.C[1] = (double)cq;
+        else if (c.c[1] == 2.0) P.C[2] = (double)cq;
+        else if (c.c[1] == 3.0) P.C[3] = (double)cq;
+        else return false;
+    } else {
+        if (c.c[4] != 0.0) return false;
+        for (int n = 0; n < 4; ++n) P.C[n] = (double)((long double)L.rho * (long double)c.c[n]);
+    }
+    const heat_law &sl = L.src_shape;
+    if (sl.kind == HEAT_LAW_CONST || (sl.kind == HEAT_LAW_POWER && sl.c[1] == 0.0)) P.src = sl.c[0];
+    else if (L.is_heater) return false;
+    P.heater = L.is_heater ? 1 : 0;
+    *out = P;
+    return true;
+}
+
+// The band kernel covers this descriptor iff it returns a variant.  Fills the per-layer table
+// and the chunk descriptors ([batch][nr/8]) when they are given.
+const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, std::vector<uint32_t> *cdesc)
+{
+    if (getenv("HEAT_VARIANT")) return nullptr;
+    if (const char *e = getenv("HEAT_KERNEL"))
+        if (strcmp(e, "line") == 0 || strcmp(e, "tma") == 0) return nullptr;
+    int G = 0, CL = 0;
+    switch (d->nr) {
+    case 512: G = 64; CL = 1; break;
+    case 1024: G = 128; CL = 1; break;
+    case 2048: G = 256; CL = 1; break;
+    case 4096: G = 256; CL = 2; break;
+    case 8192: G = 256; CL = 4; break;
+    default: return nullptr;
+    }
+    if (d->face_mode != 0 || d->nz < 4) return nullptr;
+    const int nr = d->nr, N = nr - 1;
+    if (d->r[0] != 0.0) return nullptr;
+    const long double h = (long double)d->r[N] / (long double)N;
+    for (int i = 1; i <= N; ++i)
+        if (fabsl((long double)d->r[i] - h * i) > 1e-13L * (long double)d->r[N]) return nullptr;
+    int degk = 0;
+    std::vector<PLayer> pl((size_t)d->nlayers);
+    for (int m = 0; m < d->nlayers; ++m) {
+        int dk = 0;
+        if (!to_player(d->layers[m], &pl[(size_t)m], &dk)) return nullptr;
+        degk = std::max(degk, dk);
+    }
+    const int DEGK = degk <= 2 ? 2 : 4;
+    const int cpl = nr / 8;
+    std::vector<uint32_t> cd((size_t)d->batch * cpl, 0u);
+    for (int b = 0; b < d->batch; ++b) {
+        const uint8_t *seg = d->seg_layer + (size_t)b * (nr - 1);
+        for (int c = 0; c < cpl; ++c) {
+            const int i0 = 8 * c;
+            int ks = -1;
+            for (int k = 0; k < 8; ++k) {
+                const int i = i0 + k;
+                if (i >= 1 && i < N && seg[i - 1] != seg[i]) {
+                    if (ks >= 0) return nullptr; // two interface nodes in one chunk
+                    ks = k;
+                }
+            }
+            uint32_t A, B;
+            if (ks >= 0) { A = seg[i0 + ks - 1]; B = seg[i0 + ks]; }
+            else { A = B = seg[std::min(i0, N - 1)]; }
+            uint32_t w = A | (B << 8) | ((uint32_t)(ks + 1) << 16);
+            if (c == 0) w |= BD_FIRST;
+            if (c == cpl - 1) w |= BD_LAST;
+            cd[(size_t)b * cpl + c] = w;
+        }
+    }
+    if (players) *players = pl;
+    if (cdesc) *cdesc = cd;
+    for (int v = 0; v < k_nband_variants; ++v)
+        if (k_band_variants[v].G == G && k_band_variants[v].CL == CL && k_band_variants[v].DEGK == DEGK) return &k_band_variants[v];
+    return nullptr;
+}
+
 constexpr int k_range_samples = 1025;
 
 // ---------------------------------------------------------------- workspace layout
 struct Layout {
     int nrp;
-    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, total;
+    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, total;
 };
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -178,6 +292,8 @@ Layout make_layout(const heat_desc *d, const Variant *v, const TmaVariant *tv)
     L.off_q0 = o;     o = align_up(o + sizeof(double) * (size_t)d->batch, 256);
     L.off_probes = o; o = align_up(o + sizeof(ProbeSrc) * (size_t)HEAT_MAX_PROBES, 256);
     L.off_cdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 16 + 1), 256);
+    L.off_bdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 8 + 1), 256);
+    L.off_players = o; o = align_up(o + sizeof(PLayer) * (size_t)HEAT_MAX_LAYERS, 256);
     L.total = o;
     return L;
 }
@@ -253,6 +369,9 @@ struct heat_ctx {
     std::vector<double> amp_sub; // 1 - exp(-q/k), q = 0..nsub-1, (22) P:L212 (reading G8)
     const Variant *var;
     const TmaVariant *tvar; // non-NULL: heat_step launches the TMA kernel
+    const BandVariant *bvar; // non-NULL: heat_step launches the band kernel
+    CUtensorMap btm_ld[2], btm_st[2];
+    BParams bp;
     CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
     double *field_a;
     TParams tp;
@@ -370,7 +489,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (!d->Q0) { c->P = 0; c->S = 0; }
     c->amp_sub.resize((size_t)c->nsub);
     for (int q = 0; q < c->nsub; ++q) c->amp_sub[(size_t)q] = 1.0 - std::exp(-(double)q / d->transient_k);
-    c->var = v; c->tvar = tv; c->lay = L; c->ws = (char *)workspace;
+    std::vector<PLayer> players;
+    std::vector<uint32_t> bdesc;
+    const BandVariant *bv = plan_band(d, &players, &bdesc);
+    c->var = v; c->tvar = tv; c->bvar = bv; c->lay = L; c->ws = (char *)workspace;
     c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
     c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
@@ -505,6 +627,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     UP(L.off_q0, q0, double);
     UP(L.off_probes, pr, ProbeSrc);
     UP(L.off_cdesc, cdesc, uint32_t);
+    if (bv) {
+        UP(L.off_bdesc, bdesc, uint32_t);
+        UP(L.off_players, players, PLayer);
+    }
 #undef UP
 
     // ---- initial condition (5) P:L86; Dirichlet sides hold their value from t = 0 (6);
@@ -600,6 +726,90 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         c->grid = (int)std::min<long long>(want, (long long)prop.multiProcessorCount * occ_cap);
     }
 
+
+    // ---- band kernel: launch shape, band partition, tensor maps
+    if (bv) {
+        const size_t bsmem = bv->smem_fixed + sizeof(PLayer) * (size_t)d->nlayers;
+        e = cudaFuncSetAttribute((const void *)bv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem);
+        if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", bv->name, bsmem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        int max_clusters = 0;
+        {
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * 2 * bv->CL), 1, 1);
+            cfg.blockDim = dim3(256, 1, 1);
+            cfg.dynamicSmemBytes = bsmem;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)bv->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            e = cudaOccupancyMaxActiveClusters(&max_clusters, (const void *)bv->fn, &cfg);
+            if (e != cudaSuccess || max_clusters < 1) { set_err(nullptr, "%s does not fit on the device (%s)", bv->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        }
+        if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / bv->CL);
+        // bands: every group (256/G per CTA) walks BL consecutive lines of one batch member;
+        // choose the band count per member that minimises rounds * (BL + prologue)
+        const int LPB = 256 / bv->G, Lz = nz - 2;
+        const long long slots = (long long)max_clusters * LPB;
+        long long best_cost = -1;
+        int best_BL = Lz;
+        for (int nb = 1; nb <= Lz; ++nb) {
+            const int BL = (Lz + nb - 1) / nb;
+            const int bpm = (Lz + BL - 1) / BL;
+            const long long bands = (long long)d->batch * bpm;
+            const long long rounds = (bands + slots - 1) / slots;
+            const long long cost = rounds * (BL + 3);
+            if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_BL = BL; }
+        }
+        if (const char *eb = getenv("HEAT_BAND_LINES")) best_BL = std::max(1, std::min(Lz, atoi(eb)));
+        const int bpm = (Lz + best_BL - 1) / best_BL;
+        const long long bands = (long long)d->batch * bpm;
+        const long long nclusters = std::min<long long>((bands + LPB - 1) / LPB, max_clusters);
+        c->grid = (int)nclusters * bv->CL;
+        c->smem = bsmem;
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || !sym || qres != cudaDriverEntryPointSuccess) { set_err(nullptr, "cuTensorMapEncodeTiled is unavailable (%s)", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        encode_fn encode = (encode_fn)sym;
+        const cuuint64_t gdim[2] = {16, (cuuint64_t)cells / 16};
+        const cuuint64_t gstr[1] = {128};
+        const cuuint32_t estr[2] = {1, 1};
+        const cuuint32_t box[2] = {16, (cuuint32_t)(bv->G / 2)};
+        double *lev[2] = {c->cur, c->nxt};
+        for (int q = 0; q < 2; ++q) {
+            CUresult r1 = encode(&c->btm_ld[q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, lev[q], gdim, gstr, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            CUresult r2 = encode(&c->btm_st[q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, lev[q], gdim, gstr, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) { set_err(nullptr, "cuTensorMapEncodeTiled failed (%d, %d)", (int)r1, (int)r2); return fail(HEAT_ECUDA); }
+        }
+        BParams &bp = c->bp;
+        memset(&bp, 0, sizeof bp);
+        bp.cdesc = (const uint32_t *)(c->ws + L.off_bdesc);
+        bp.players = (const PLayer *)(c->ws + L.off_players);
+        bp.ezm = (const double *)(c->ws + L.off_ezm);
+        bp.ezp = (const double *)(c->ws + L.off_ezp);
+        bp.Q0 = (const double *)(c->ws + L.off_q0);
+        bp.probes = (const ProbeSrc *)(c->ws + L.off_probes);
+        {
+            const long double h = ((long double)r[N] - (long double)r[0]) / (long double)N;
+            bp.g0 = (double)(1.0L / (h * h));
+        }
+        const bool din = d->r_in.kind == HEAT_BC_DIRICHLET, dout = d->r_out.kind == HEAT_BC_DIRICHLET;
+        bp.rin_om = din ? 1.0 : 0.0; bp.rin_be = din ? d->r_in.value : 0.0;
+        bp.rout_a = dout ? 0.0 : 1.0; bp.rout_w = dout ? 1.0 : 0.0; bp.rout_f = dout ? d->r_out.value : 0.0;
+        bp.nr = nr; bp.nz = nz; bp.batch = d->batch; bp.nlayers = d->nlayers; bp.nprobes = d->nprobes;
+        bp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
+        bp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
+        bp.rpl = nr / 16; bp.BL = best_BL; bp.bands_per_member = bpm; bp.total_bands = (int)bands;
+    }
+
     KParams &k = c->kp;
     memset(&k, 0, sizeof k);
     k.ga = (const double *)(c->ws + L.off_ga);
@@ -647,7 +857,25 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
                 c->rec_dropped += 1;
             }
         }
-        if (c->tvar) {
+        if (c->bvar) {
+            const int q = (c->cur == c->field_a) ? 0 : 1;
+            BParams &bp = c->bp;
+            bp.tm_ld = c->btm_ld[q];
+            bp.tm_st = c->btm_st[1 - q];
+            bp.Told = c->cur;
+            bp.inv_tau = k.inv_tau; bp.amp = k.amp; bp.probe_out = k.probe_out;
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)c->grid, 1, 1);
+            cfg.blockDim = dim3(256, 1, 1);
+            cfg.dynamicSmemBytes = c->smem;
+            cfg.stream = st;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)c->bvar->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->bvar->fn, bp));
+        } else if (c->tvar) {
             const int q = (c->cur == c->field_a) ? 0 : 1;
             c->tp.tm_ld = c->tm_ld[q];
             c->tp.tm_st = c->tm_st[1 - q];
@@ -718,7 +946,7 @@ heat_status heat_probe(heat_ctx *c, double *dst_host, int64_t max, int64_t *n_wr
 
 int64_t heat_step_index(const heat_ctx *c) { return c ? c->step : -1; }
 int64_t heat_launch_count(const heat_ctx *c) { return c ? c->launches : -1; }
-const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->tvar ? c->tvar->name : c->var->name) : ""; }
+const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->bvar ? c->bvar->name : c->tvar ? c->tvar->name : c->var->name) : ""; }
 const char *heat_last_error(const heat_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
 void heat_destroy(heat_ctx *c) { delete c; }
 

@@ -1,0 +1,553 @@
+// heat_band_kernel.cuh -- third-generation fused time-step kernel for sm_100a ("band kernel")
+// (same arithmetic contract as heat_line_kernel.cuh).
+//
+// What differs from heat_tma_kernel.cuh (v2) and from the paper's one-work-item-per-line
+// kernel:
+//   * A CTA group owns a BAND of consecutive z-lines and walks it line by line.  Each line of the
+//     current level is brought into shared memory exactly once (TMA, SWIZZLE_128B, prefetched two
+//     lines ahead through a ring of four slots), so L2 -> SM traffic is 8 B per cell instead of 24.
+//   * The explicit axial face flux lambda_{i,j+1/2} (T_{i,j+1} - T_{i,j}) of eq. (11) P:L125 is
+//     computed once per face: line j computes its upper flux, keeps it in a thread-private shared
+//     slot, and line j+1 reuses it (with the opposite sign) as its lower flux.
+//   * A thread owns 8 consecutive nodes; the sweep coefficients (alpha, beta, gamma) of eq. (12)
+//     P:L133-136 stay in REGISTERS between the forward sweep and the back substitution (14).
+//   * The row arithmetic is branch free across materials: every property law is a polynomial
+//     (optionally times a square root) whose coefficients live in per-thread registers, loaded
+//     once per band, so warps that span two layers do not serialise.  r-boundary rows (15) are
+//     selects at fixed positions; only the thread that holds an interface node (18) takes a short
+//     fix-up branch.
+//   * The reduced system (one row per thread) is solved as in v2: shuffle PCR inside a warp,
+//     one separator row per warp, separators exchanged through (distributed) shared memory and
+//     solved by PCR in one warp.  Lines longer than 2048 nodes span a cluster of 2 or 4 CTAs.
+// The kernel covers uniform r grids starting at r = 0 with nr in {512,1024,2048,4096,8192},
+// laws CONST / POWER(p in {0,.5,1,1.5,2,3}) / POLY, lambda at the mean temperature (face_mode 0)
+// and a temperature-independent source shape; heat_create picks v2 / v1 for everything else.
+// "P:Lnnn" cites a line of the paper text; readings G1..G22 are listed in DESIGN.md.
+#pragma once
+#include <cuda.h>
+
+#include "heat_band_params.cuh"
+#include "heat_tma_kernel.cuh"
+
+namespace heat {
+
+__device__ __forceinline__ void bulk_load_16(uint32_t dst, const void *src, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 16, [%2];"
+                 ::"r"(dst), "l"(src), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
+
+// reciprocal: MUFU.RCP64H seed (>= 20 bits) + one cubic step e -> e^3: ~2^-60 before rounding
+__device__ __forceinline__ double rcp_cubic(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
+}
+
+template <int DEGK>
+struct BCoef {
+    double K[DEGK + 1];
+    double C[4]; // times 1/tau
+    double qs;   // Q0 nu p^2 s  (2)-(4),(22); 0 outside the heater
+    bool sq;
+};
+
+template <int DEGK>
+__device__ __forceinline__ BCoef<DEGK> load_coef(const PLayer &L, double inv_tau, double qa)
+{
+    BCoef<DEGK> c;
+#pragma unroll
+    for (int n = 0; n <= DEGK; ++n) c.K[n] = L.K[n];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) c.C[n] = L.C[n] * inv_tau;
+    c.qs = L.heater ? qa * L.src : 0.0;
+    c.sq = (L.sqrtk != 0);
+    return c;
+}
+
+// lambda at a face from s = Ta + Tb; anysq is warp-uniform
+template <int DEGK>
+__device__ __forceinline__ double lam_eval(const BCoef<DEGK> &c, bool anysq, double s)
+{
+    double v = c.K[DEGK];
+#pragma unroll
+    for (int n = DEGK - 1; n >= 0; --n) v = fma(v, s, c.K[n]);
+    if (anysq) {
+        const double r = sqrt(s);
+        v = c.sq ? v * r : v;
+    }
+    return v;
+}
+
+template <int DEGK>
+__device__ __forceinline__ double cap_eval(const BCoef<DEGK> &c, double T)
+{
+    double v = c.C[3];
+    v = fma(v, T, c.C[2]);
+    v = fma(v, T, c.C[1]);
+    v = fma(v, T, c.C[0]);
+    return v;
+}
+
+// One row pushed through the sweep (12) P:L133-136 in its all-positive form.  The row is
+//   -a x_{i-1} + (a + c + w) x_i - c x_{i+1} = f,      a, c, w >= 0,
+// a = cfL, c = cfR, and with om = 1 - alpha_{i-1}:  den = w + c + a om,  alpha_i = c / den,
+// 1 - alpha_i = (w + a om) / den,  beta_i = (f + a beta_{i-1}) / den,  gamma_i = a gamma_{i-1} / den.
+struct SweepState {
+    double cfL, om, be, gm;
+};
+
+__device__ __forceinline__ void sweep_row(SweepState &s, double cfR, double w, double f, double &al)
+{
+    const double g = fma(s.cfL, s.om, w);
+    const double inv = rcp_cubic(g + cfR);
+    const double tA = s.cfL * inv;
+    al = cfR * inv;
+    s.om = g * inv;
+    s.be = fma(tA, s.be, f * inv);
+    s.gm = tA * s.gm;
+    s.cfL = cfR;
+}
+
+// A regular row (13) P:L140-145 of the uniform r grid, scaled by i = r_i / h:
+//   cfR = (i + 1/2) g0 lambda_{i+1/2,j},  w = i rho c / tau,  f = w T + i (Lambda_j[T] + X),
+// Lambda_j[T] (11) P:L125 = ezp fU - ezm fD with the face fluxes fU, fD = lambda (T' - T).
+template <int DEGK>
+__device__ __forceinline__ void regular_row(const BCoef<DEGK> &c, bool anysq, double T, double Tr, double Tu, double fD,
+                                            double fi, double g0, double ezp, double ezm, double &cfR, double &w,
+                                            double &f, double &fU)
+{
+    cfR = lam_eval<DEGK>(c, anysq, T + Tr) * fma(g0, fi, 0.5 * g0);
+    w = cap_eval<DEGK>(c, T) * fi;
+    fU = lam_eval<DEGK>(c, anysq, T + Tu) * (Tu - T);
+    double lz = fma(ezp, fU, c.qs);
+    lz = fma(-ezm, fD, lz);
+    f = fma(w, T, fi * lz);
+}
+
+// the same laws straight from the shared-memory layer table (fix-up path: short live ranges)
+template <int DEGK>
+__device__ __noinline__ double lam_smem(const PLayer *L, double s)
+{
+    double v = L->K[DEGK];
+#pragma unroll
+    for (int n = DEGK - 1; n >= 0; --n) v = fma(v, s, L->K[n]);
+    if (L->sqrtk) v *= sqrt(s);
+    return v;
+}
+static __device__ __noinline__ double cap_smem(const PLayer *L, double T, double inv_tau)
+{
+    double v = L->C[3];
+    v = fma(v, T, L->C[2]);
+    v = fma(v, T, L->C[1]);
+    v = fma(v, T, L->C[0]);
+    return v * inv_tau;
+}
+
+
+// G  = threads of this CTA that work on one line (64, 128 or 256); CTA = 256 threads.
+// CL = cluster size; CL > 1 needs G == 256: the line has 256*CL threads, rank c owns nodes
+//      [2048c, 2048c + 2048).
+// DEGK = degree of the lambda polynomials.
+template <int G, int CL, int DEGK>
+__global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant__ BParams p)
+{
+    using Cfg = BandCfg<G, CL>;
+    constexpr int SLOT = Cfg::SLOT;
+    constexpr int LPB = Cfg::LPB;
+    constexpr int WG = Cfg::WG;
+    constexpr int NSEP = Cfg::NSEP;
+    constexpr uint32_t FULL = 0xffffffffu;
+    static_assert(CL == 1 || G == 256, "a cluster line needs whole CTAs");
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char *gbase = smem_raw + (sbase - smem_u32(smem_raw));
+    double *pub = reinterpret_cast<double *>(gbase + Cfg::OFF_PUB);   // [2][NSEP][PUB]
+    double *ysep = reinterpret_cast<double *>(gbase + Cfg::OFF_YSEP); // [NSEP]
+    PLayer *lay = reinterpret_cast<PLayer *>(gbase + Cfg::OFF_LAY);
+    const uint32_t mbar_a = sbase + Cfg::OFF_MBAR;
+    const uint32_t pub_a = sbase + Cfg::OFF_PUB;
+    const uint32_t halo_a = sbase + Cfg::OFF_HALO;
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int warp = tid >> 5;
+    const int crank = (CL > 1) ? (int)cluster_ctarank() : 0;
+    const int grp = tid / G;            // group (line) within the CTA
+    const int tg = tid % G;             // thread within the CTA's part of the line
+    const int t = crank * G + tg;       // thread within the line
+    const int i0 = t * 8;
+    const int wig = t >> 5;             // warp within the line
+    const int gs = crank * 8 + warp;    // this warp's separator slot
+    const int trow = tid >> 1, half = tid & 1, sw = trow & 7;
+    // byte offsets inside a slot: own 16-byte chunks q = 0..3, and the two r neighbours
+    const uint32_t rowo = (uint32_t)trow * 128u;
+    uint32_t co[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) co[q] = rowo + (uint32_t)((((half << 2) | q) ^ sw) << 4);
+    const uint32_t hlo = half ? (rowo + (uint32_t)((3 ^ sw) << 4) + 8u)
+                              : (rowo - 128u + (uint32_t)((7 ^ ((trow - 1) & 7)) << 4) + 8u);
+    const uint32_t hro = half ? (rowo + 128u + (uint32_t)((0 ^ ((trow + 1) & 7)) << 4))
+                              : (rowo + (uint32_t)((4 ^ sw) << 4));
+    const bool edgeL = (tg == 0), edgeR = (tg == G - 1);
+
+    for (int q = tid; q < p.nlayers * (int)(sizeof(PLayer) / sizeof(int)); q += Cfg::NT)
+        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.players)[q];
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < 4; ++s) mbar_init(mbar_a + 8u * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (CL > 1) { cluster_arrive(); cluster_wait(); }
+
+    const int nr = p.nr, nz = p.nz, BL = p.BL, bpm = p.bands_per_member;
+    const int cluster_id = blockIdx.x / CL, nclusters = gridDim.x / CL;
+    const double g0 = p.g0;
+    const double fi0 = (double)i0;
+    uint32_t qbase = 0;   // load sequence number of line offset -1 of this round
+    uint32_t pubpar = 0;  // parity of the separator exchange buffer
+
+    // line offset L (-1 .. BL) of this CTA's bands -> TMA loads into slot (qbase+L+1)&3
+    auto issue_loads = [&](int round, int L) {
+        const uint32_t q = qbase + (uint32_t)(L + 1);
+        const uint32_t slot = sbase + (q & 3u) * (uint32_t)SLOT;
+        const uint32_t bar = mbar_a + 8u * (q & 3u);
+        uint32_t bytes = 0;
+        int R[LPB];
+#pragma unroll
+        for (int g = 0; g < LPB; ++g) {
+            const int band = (round * nclusters + cluster_id) * LPB + g;
+            R[g] = -1;
+            if (band < p.total_bands) {
+                const int b = band / bpm, j0 = 1 + (band - b * bpm) * BL;
+                const int j1 = min(j0 + BL, nz - 1);
+                const int j = j0 + L;
+                if (j <= j1) {
+                    R[g] = (b * nz + j) * p.rpl + crank * (G / 2);
+                    bytes += (uint32_t)(G * 64);
+                }
+            }
+        }
+        if (CL > 1 && R[0] >= 0) bytes += (crank > 0 ? 16u : 0u) + (crank < CL - 1 ? 16u : 0u);
+        mbar_expect_tx(bar, bytes);
+#pragma unroll
+        for (int g = 0; g < LPB; ++g)
+            if (R[g] >= 0) tma_load_2d(slot + (uint32_t)(g * G * 64), &p.tm_ld, 0, R[g], bar);
+        if (CL > 1 && R[0] >= 0) {
+            const double *row0 = p.Told + (size_t)R[0] * 16;
+            if (crank > 0) bulk_load_16(halo_a + (q & 3u) * 32u, row0 - 2, bar);
+            if (crank < CL - 1) bulk_load_16(halo_a + (q & 3u) * 32u + 16u, row0 + (size_t)(G / 2) * 16, bar);
+        }
+    };
+    auto wait_slot = [&](int L) {
+        const uint32_t q = qbase + (uint32_t)(L + 1);
+        while (!mbar_try_wait(mbar_a + 8u * (q & 3u), (q >> 2) & 1u)) {}
+    };
+    // line offset L of this CTA's bands -> TMA stores of the new level from its slot
+    auto issue_stores = [&](int round, int L) {
+        const uint32_t q = qbase + (uint32_t)(L + 1);
+        const uint32_t slot = sbase + (q & 3u) * (uint32_t)SLOT;
+#pragma unroll
+        for (int g = 0; g < LPB; ++g) {
+            const int band = (round * nclusters + cluster_id) * LPB + g;
+            if (band >= p.total_bands) continue;
+            const int b = band / bpm, j0 = 1 + (band - b * bpm) * BL;
+            const int j1 = min(j0 + BL, nz - 1);
+            const int j = j0 + L;
+            if (j >= j1) continue;
+            const int Rg = (b * nz + j) * p.rpl + crank * (G / 2);
+            const uint32_t src = slot + (uint32_t)(g * G * 64);
+            tma_store_2d(&p.tm_st, 0, Rg, src);
+            // Neumann z lines copy their neighbour (reading G16)
+            if (j == 1 && p.z_lo_neumann) tma_store_2d(&p.tm_st, 0, Rg - p.rpl, src);
+            if (j == nz - 2 && p.z_hi_neumann) tma_store_2d(&p.tm_st, 0, Rg + p.rpl, src);
+        }
+        tma_commit();
+    };
+
+    for (int round = 0; (round * nclusters) * LPB < p.total_bands; ++round) {
+        const int band = (round * nclusters + cluster_id) * LPB + grp;
+        const bool live = band < p.total_bands;
+        const int bandc = live ? band : p.total_bands - 1;
+        const int b = bandc / bpm;
+        const int j0 = 1 + (bandc - b * bpm) * BL;
+        const int j1 = min(j0 + BL, nz - 1);
+
+        // ---- per-thread constants of this band: laws of the chunk's layer, row flags
+        const uint32_t cd = __ldg(p.cdesc + (size_t)b * (nr / 8) + t);
+        const double qa = __ldg(p.Q0 + b) * p.amp; // Q0 nu(t_k) p^2(t_k), (2)-(4),(22)
+        const BCoef<DEGK> cA = load_coef<DEGK>(lay[cd & 0xffu], p.inv_tau, qa);
+        const int ks = (int)((cd >> 16) & 0xfu) - 1;
+        const bool first = (cd & BD_FIRST) != 0, last = (cd & BD_LAST) != 0;
+        const bool anysq = __any_sync(FULL, cA.sq);
+
+        if (tid == 32) { // thread 32 issues every TMA load and store (bulk groups are per thread)
+            issue_loads(round, -1);
+            issue_loads(round, 0);
+            issue_loads(round, 1);
+        }
+        wait_slot(-1);
+        wait_slot(0);
+
+        // ---- prologue: the flux through the faces between lines j0-1 and j0
+        {
+            const uint32_t sd = sbase + ((qbase + 0u) & 3u) * (uint32_t)SLOT;
+            const uint32_t sc = sbase + ((qbase + 1u) & 3u) * (uint32_t)SLOT;
+            const PLayer *LB = lay + ((cd >> 8) & 0xffu);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const double2 td = lds128(sd + co[q]);
+                const double2 tc = lds128(sc + co[q]);
+                double f0 = lam_eval<DEGK>(cA, anysq, tc.x + td.x) * (tc.x - td.x);
+                double f1 = lam_eval<DEGK>(cA, anysq, tc.y + td.y) * (tc.y - td.y);
+                if (ks >= 0) { // rows above the interface node belong to layer B
+                    if (2 * q > ks) f0 = lam_smem<DEGK>(LB, tc.x + td.x) * (tc.x - td.x);
+                    if (2 * q + 1 > ks) f1 = lam_smem<DEGK>(LB, tc.y + td.y) * (tc.y - td.y);
+                }
+                sts128(sbase + Cfg::OFF_FLUX + co[q], f0, f1);
+            }
+        }
+
+        for (int L = 0; L < BL; ++L) {
+            const uint32_t q = qbase + (uint32_t)(L + 1);
+            const uint32_t sc = sbase + (q & 3u) * (uint32_t)SLOT;        // line j   (centre)
+            const uint32_t su = sbase + ((q + 1u) & 3u) * (uint32_t)SLOT; // line j+1 (up)
+            const uint32_t fr = sbase + Cfg::OFF_FLUX + (uint32_t)(L & 1) * (uint32_t)SLOT;       // fD
+            const uint32_t fw = sbase + Cfg::OFF_FLUX + (uint32_t)((L & 1) ^ 1) * (uint32_t)SLOT; // fU
+            const int j = j0 + L;
+            const bool line_live = live && (j < j1);
+            const int jc = min(j, nz - 2);
+            if (tid == 32 && L + 2 <= BL) {
+                tma_wait_read0(); // the store that last used the prefetch slot has read it
+                issue_loads(round, L + 2);
+            }
+            const double ezm = __ldg(p.ezm + jc), ezp = __ldg(p.ezp + jc);
+            wait_slot(L + 1);
+
+            // ---- line j of the current level: the two r neighbours of the thread's 8 nodes
+            double hl, hr;
+            {
+                const double2 v0 = lds128(sc + co[0]);
+                const double2 v3 = lds128(sc + co[3]);
+                hl = v0.x; hr = v3.y;
+            }
+            if (!edgeL) hl = lds64(sc + hlo);
+            else if (CL > 1 && crank > 0) hl = lds64(halo_a + (q & 3u) * 32u + 8u);
+            if (!edgeR) hr = lds64(sc + hro);
+            else if (CL > 1 && crank < CL - 1) hr = lds64(halo_a + (q & 3u) * 32u + 16u);
+
+            // ---- level 1: assemble (13)/(15) and sweep (12) the thread's 8 rows
+            double al[8], be[8], gm[8];
+            {
+                SweepState st;
+                st.om = 1.0; st.be = 0.0; st.gm = 1.0;
+                double2 tl = lds128(sc + co[0]);
+                st.cfL = lam_eval<DEGK>(cA, anysq, hl + tl.x) * fma(g0, fi0, -0.5 * g0); // face i0 - 1/2
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) {
+                    double2 tn;
+                    if (qq < 3) tn = lds128(sc + co[qq < 3 ? qq + 1 : 3]);
+                    else tn = make_double2(hr, hr);
+                    const double2 tu = lds128(su + co[qq]);
+                    const double2 fd = lds128(fr + co[qq]);
+                    double fu[2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int k = 2 * qq + e;
+                        double cfR, w, f;
+                        regular_row<DEGK>(cA, anysq, e ? tl.y : tl.x, e ? tn.x : tl.y, e ? tu.y : tu.x, e ? fd.y : fd.x,
+                                          fi0 + (double)k, g0, ezp, ezm, cfR, w, f, fu[e]);
+                        if (k == 7) { // r_out boundary row (15),(17) P:L158-174
+                            st.cfL = last ? p.rout_a : st.cfL;
+                            cfR = last ? 0.0 : cfR;
+                            w = last ? p.rout_w : w;
+                            f = last ? p.rout_f : f;
+                        }
+                        sweep_row(st, cfR, w, f, al[k]);
+                        if (k == 0) { // r_in boundary row (15),(16) P:L158-169
+                            al[0] = first ? 1.0 - p.rin_om : al[0];
+                            st.om = first ? p.rin_om : st.om;
+                            st.be = first ? p.rin_be : st.be;
+                            st.gm = first ? 0.0 : st.gm;
+                        }
+                        be[k] = st.be; gm[k] = st.gm;
+                    }
+                    sts128(fw + co[qq], fu[0], fu[1]);
+                    tl = tn;
+                }
+            }
+
+            // ---- fix-up: the chunk holds an interface node (18)-(20) P:L176-192 at row ks;
+            //      rows above it belong to layer B.  Redo rows ks..7 (rare, one lane per interface).
+            if (__builtin_expect(ks >= 0, 0)) {
+                const PLayer *LA = lay + (cd & 0xffu), *LB = lay + ((cd >> 8) & 0xffu);
+                const double qsB = LB->heater ? qa * LB->src : 0.0;
+                SweepState s2;
+                s2.om = 1.0; s2.be = 0.0; s2.gm = 1.0; s2.cfL = 0.0;
+#pragma unroll
+                for (int k = 0; k < 7; ++k)
+                    if (k == ks - 1) { s2.om = 1.0 - al[k]; s2.be = be[k]; s2.gm = gm[k]; }
+                double Tp = hl;
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) {
+                    const double2 tc = lds128(sc + co[qq]);
+                    const double tnx = (qq < 3) ? lds64(sc + co[qq < 3 ? qq + 1 : 3]) : hr;
+                    const double2 tu = lds128(su + co[qq]);
+                    const double2 fd = lds128(fr + co[qq]);
+                    double2 fu = lds128(fw + co[qq]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int k = 2 * qq + e;
+                        const double Tl_ = e ? tc.x : Tp, T_ = e ? tc.y : tc.x, Tr_ = e ? tnx : tc.y;
+                        const double Tu_ = e ? tu.y : tu.x, fD_ = e ? fd.y : fd.x;
+                        if (k < ks) continue;
+                        double cfR, w, f;
+                        if (k == ks) {
+                            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0,
+                            // lam* at T_{i*,j}; new level (reading G7)
+                            s2.cfL = lam_smem<DEGK>(LA, T_ + T_);
+                            cfR = lam_smem<DEGK>(LB, T_ + T_);
+                            w = 0.0; f = 0.0;
+                        } else {
+                            const double fi = fi0 + (double)k;
+                            s2.cfL = lam_smem<DEGK>(LB, Tl_ + T_) * fma(g0, fi, -0.5 * g0);
+                            cfR = lam_smem<DEGK>(LB, T_ + Tr_) * fma(g0, fi, 0.5 * g0);
+                            w = cap_smem(LB, T_, p.inv_tau) * fi;
+                            const double fuk = lam_smem<DEGK>(LB, T_ + Tu_) * (Tu_ - T_);
+                            double lz = fma(ezp, fuk, qsB);
+                            lz = fma(-ezm, fD_, lz);
+                            f = fma(w, T_, fi * lz);
+                            if (e) fu.y = fuk; else fu.x = fuk;
+                            if (k == 7 && last) { s2.cfL = p.rout_a; cfR = 0.0; w = p.rout_w; f = p.rout_f; }
+                        }
+                        sweep_row(s2, cfR, w, f, al[k]);
+                        be[k] = s2.be; gm[k] = s2.gm;
+                    }
+                    sts128(fw + co[qq], fu.x, fu.y);
+                    Tp = tc.y;
+                }
+            }
+
+            // ---- x_first = P x_last + Q + S u from the stored sweep coefficients
+            double P = al[6], Q = be[6], S = gm[6];
+#pragma unroll
+            for (int k = 5; k >= 0; --k) {
+                Q = fma(al[k], Q, be[k]);
+                S = fma(al[k], S, gm[k]);
+                P = P * al[k];
+            }
+
+            // ---- reduced row of this thread: a*y_{t-1} + y_t + c*y_{t+1} = d  (y = x of the last row)
+            double Pn = __shfl_down_sync(FULL, P, 1);
+            double Qn = __shfl_down_sync(FULL, Q, 1);
+            double Sn = __shfl_down_sync(FULL, S, 1);
+            if (lane == 31) { Pn = 0.0; Qn = 0.0; Sn = 0.0; }
+            Row3 row;
+            {
+                const double r = rcp_cubic(fma(-al[7], Sn, 1.0));
+                row.a = -gm[7] * r;
+                row.c = -al[7] * Pn * r;
+                row.d = fma(al[7], Qn, be[7]) * r;
+            }
+            // ---- level 2: PCR over lanes 0..30; lane 31 is the warp's separator
+            const Row3 rp = pcr_segment<32>(row, lane, 0, 30);
+            Row3 r30;
+            r30.a = __shfl_sync(FULL, rp.a, 30);
+            r30.c = __shfl_sync(FULL, rp.c, 30);
+            r30.d = __shfl_sync(FULL, rp.d, 30);
+            {
+                const uint32_t slot = pub_a + (uint32_t)((pubpar * NSEP + gs) * Cfg::PUB) * 8u;
+                if (lane == 0 || lane == 31) {
+                    const uint32_t s6 = slot + (lane == 31 ? 48u : 0u);
+                    const double v0 = lane == 31 ? al[7] : P, v1 = lane == 31 ? be[7] : Q, v2 = lane == 31 ? gm[7] : S;
+                    const double v3 = lane == 31 ? r30.a : rp.a, v4 = lane == 31 ? r30.c : rp.c, v5 = lane == 31 ? r30.d : rp.d;
+                    if (CL > 1) {
+#pragma unroll
+                        for (int rk = 0; rk < CL; ++rk) {
+                            const uint32_t ra = map_to_rank(s6, (uint32_t)rk);
+                            st_cluster_f64(ra, v0); st_cluster_f64(ra + 8, v1); st_cluster_f64(ra + 16, v2);
+                            st_cluster_f64(ra + 24, v3); st_cluster_f64(ra + 32, v4); st_cluster_f64(ra + 40, v5);
+                        }
+                    } else {
+                        sts64(s6, v0); sts64(s6 + 8, v1); sts64(s6 + 16, v2);
+                        sts64(s6 + 24, v3); sts64(s6 + 32, v4); sts64(s6 + 40, v5);
+                    }
+                }
+            }
+            if (CL > 1) { cluster_arrive(); cluster_wait(); } else __syncthreads();
+            // ---- level 3: warp 0 builds every separator row and solves them (PCR per line)
+            if (warp == 0) {
+                const bool in3 = lane < NSEP;
+                const int s = in3 ? lane : 0;
+                const double *D = pub + (pubpar * NSEP + s) * Cfg::PUB;
+                const bool has_next = ((s % WG) + 1 < WG);
+                const double *Dn = D + (has_next ? Cfg::PUB : 0);
+                const double sal = D[6], sbe = D[7], sgm = D[8];
+                Row3 l30; l30.a = D[9]; l30.c = D[10]; l30.d = D[11];
+                Row3 nx; nx.a = nx.c = nx.d = 0.0;
+                double Pw = 0.0, Qw = 0.0, Sw = 0.0;
+                if (has_next) { Pw = Dn[0]; Qw = Dn[1]; Sw = Dn[2]; nx.a = Dn[3]; nx.c = Dn[4]; nx.d = Dn[5]; }
+                Row3 me;
+                const double r = rcp_cubic(fma(-sal, Sw, 1.0));
+                me.a = -sgm * r;
+                me.c = -sal * Pw * r;
+                me.d = fma(sal, Qw, sbe) * r;
+                Row3 s3 = pcr_combine(me, l30, true, nx, has_next);
+                s3 = pcr_segment<WG>(s3, s % WG, 0, WG - 1);
+                if (in3) ysep[s] = s3.d;
+            } else if (tid == 32 && L > 0) {
+                issue_stores(round, L - 1); // every thread passed the barrier after writing line L-1
+            }
+            __syncthreads();
+            pubpar ^= 1u;
+            double y, u;
+            {
+                const double Vs = ysep[gs];
+                const double U = (wig > 0) ? ysep[gs - 1] : 0.0;
+                y = (lane == 31) ? Vs : fma(-rp.c, Vs, fma(-rp.a, U, rp.d));
+                u = __shfl_up_sync(FULL, y, 1);
+                if (lane == 0) u = U;
+            }
+
+            // ---- back substitution (14) P:L150; the new level replaces line j in its slot
+            double x[8];
+            x[7] = y;
+#pragma unroll
+            for (int k = 6; k >= 0; --k) x[k] = fma(al[k], x[k + 1], fma(gm[k], u, be[k]));
+#pragma unroll
+            for (int qq = 0; qq < 4; ++qq) sts128(sc + co[qq], x[2 * qq], x[2 * qq + 1]);
+            fence_proxy_async();
+
+            // ---- probes: T of the new level at (i_p, j_p)
+            if (p.probe_out != nullptr && line_live) {
+                for (int pq = 0; pq < p.nprobes; ++pq) {
+                    const ProbeSrc ps = p.probes[pq];
+                    if (ps.i < i0 || ps.i >= i0 + 8) continue;
+                    if (ps.is_static) {
+                        if (j == 1) p.probe_out[b * p.nprobes + pq] = p.Told[((size_t)b * nz + ps.j_store) * nr + ps.i];
+                    } else if (ps.j_src == j) {
+                        double v = 0.0;
+#pragma unroll
+                        for (int k = 0; k < 8; ++k)
+                            if (i0 + k == ps.i) v = x[k];
+                        p.probe_out[b * p.nprobes + pq] = v;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        if (tid == 32) issue_stores(round, BL - 1);
+        qbase += (uint32_t)(BL + 2);
+        if (tid == 32) tma_wait_read0(); // the next round's loads reuse the slots
+        __syncthreads();
+    }
+    if (tid == 32) tma_wait_all0();
+    if (CL > 1) { cluster_arrive(); cluster_wait(); }
+}
+
+} // namespace heat

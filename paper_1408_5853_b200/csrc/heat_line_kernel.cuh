@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
 }
 
 // ---------------------------------------------------------------- fp64 FMA peak probe
-__global__ void fp64_peak_kernel(double *out, long long iters, double a, double b)
+static __global__ void fp64_peak_kernel(double *out, long long iters, double a, double b)
 {
     double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
     for (long long it = 0; it < iters; ++it) {
