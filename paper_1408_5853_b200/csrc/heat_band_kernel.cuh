@@ -48,6 +48,20 @@ __device__ __forceinline__ double rcp_cubic(double x)
     return fma(y, t, y);
 }
 
+// square root for lambda ~ T^(p+1/2): MUFU.RSQ64H seed (>= 20 bits) + two coupled Newton steps
+// (g -> sqrt s, hy -> 1/(2 sqrt s)); relative error ~2^-52, no special cases (s > 0 here)
+__device__ __forceinline__ double sqrt_pos(double s)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+    double g = s * y, hy = 0.5 * y;
+    double r = fma(-hy, g, 0.5);
+    g = fma(g, r, g);
+    hy = fma(hy, r, hy);
+    r = fma(-hy, g, 0.5);
+    return fma(g, r, g);
+}
+
 template <int DEGK>
 struct BCoef {
     double K[DEGK + 1];
@@ -77,7 +91,7 @@ __device__ __forceinline__ double lam_eval(const BCoef<DEGK> &c, bool anysq, dou
 #pragma unroll
     for (int n = DEGK - 1; n >= 0; --n) v = fma(v, s, c.K[n]);
     if (anysq) {
-        const double r = sqrt(s);
+        const double r = sqrt_pos(s);
         v = c.sq ? v * r : v;
     }
     return v;
@@ -128,26 +142,6 @@ __device__ __forceinline__ void regular_row(const BCoef<DEGK> &c, bool anysq, do
     lz = fma(-ezm, fD, lz);
     f = fma(w, T, fi * lz);
 }
-
-// the same laws straight from the shared-memory layer table (fix-up path: short live ranges)
-template <int DEGK>
-__device__ __noinline__ double lam_smem(const PLayer *L, double s)
-{
-    double v = L->K[DEGK];
-#pragma unroll
-    for (int n = DEGK - 1; n >= 0; --n) v = fma(v, s, L->K[n]);
-    if (L->sqrtk) v *= sqrt(s);
-    return v;
-}
-static __device__ __noinline__ double cap_smem(const PLayer *L, double T, double inv_tau)
-{
-    double v = L->C[3];
-    v = fma(v, T, L->C[2]);
-    v = fma(v, T, L->C[1]);
-    v = fma(v, T, L->C[0]);
-    return v * inv_tau;
-}
-
 
 // G  = threads of this CTA that work on one line (64, 128 or 256); CTA = 256 threads.
 // CL = cluster size; CL > 1 needs G == 256: the line has 256*CL threads, rank c owns nodes
@@ -208,7 +202,7 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
     const int nr = p.nr, nz = p.nz, BL = p.BL, bpm = p.bands_per_member;
     const int cluster_id = blockIdx.x / CL, nclusters = gridDim.x / CL;
     const double g0 = p.g0;
-    const double fi0 = (double)i0;
+    double fi0 = (double)i0;
     uint32_t qbase = 0;   // load sequence number of line offset -1 of this round
     uint32_t pubpar = 0;  // parity of the separator exchange buffer
 
@@ -281,10 +275,12 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
         // ---- per-thread constants of this band: laws of the chunk's layer, row flags
         const uint32_t cd = __ldg(p.cdesc + (size_t)b * (nr / 8) + t);
         const double qa = __ldg(p.Q0 + b) * p.amp; // Q0 nu(t_k) p^2(t_k), (2)-(4),(22)
-        const BCoef<DEGK> cA = load_coef<DEGK>(lay[cd & 0xffu], p.inv_tau, qa);
+        BCoef<DEGK> cA = load_coef<DEGK>(lay[cd & 0xffu], p.inv_tau, qa);
         const int ks = (int)((cd >> 16) & 0xfu) - 1;
         const bool first = (cd & BD_FIRST) != 0, last = (cd & BD_LAST) != 0;
-        const bool anysq = __any_sync(FULL, cA.sq);
+        // a chunk with an interface node switches to the laws of layer B behind it (warp-uniform flag)
+        const bool anysp = __any_sync(FULL, ks >= 0);
+        const bool anysq = __any_sync(FULL, cA.sq || (ks >= 0 && lay[(cd >> 8) & 0xffu].sqrtk != 0));
 
         if (tid == 32) { // thread 32 issues every TMA load and store (bulk groups are per thread)
             issue_loads(round, -1);
@@ -298,18 +294,19 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
         {
             const uint32_t sd = sbase + ((qbase + 0u) & 3u) * (uint32_t)SLOT;
             const uint32_t sc = sbase + ((qbase + 1u) & 3u) * (uint32_t)SLOT;
-            const PLayer *LB = lay + ((cd >> 8) & 0xffu);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const double2 td = lds128(sd + co[q]);
                 const double2 tc = lds128(sc + co[q]);
-                double f0 = lam_eval<DEGK>(cA, anysq, tc.x + td.x) * (tc.x - td.x);
-                double f1 = lam_eval<DEGK>(cA, anysq, tc.y + td.y) * (tc.y - td.y);
-                if (ks >= 0) { // rows above the interface node belong to layer B
-                    if (2 * q > ks) f0 = lam_smem<DEGK>(LB, tc.x + td.x) * (tc.x - td.x);
-                    if (2 * q + 1 > ks) f1 = lam_smem<DEGK>(LB, tc.y + td.y) * (tc.y - td.y);
+                double fl[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int k = 2 * q + e;
+                    if (anysp && k == ks) cA = load_coef<DEGK>(lay[(cd >> 8) & 0xffu], p.inv_tau, qa);
+                    const double a_ = e ? tc.y : tc.x, d_ = e ? td.y : td.x;
+                    fl[e] = lam_eval<DEGK>(cA, anysq, a_ + d_) * (a_ - d_);
                 }
-                sts128(sbase + Cfg::OFF_FLUX + co[q], f0, f1);
+                sts128(sbase + Cfg::OFF_FLUX + co[q], fl[0], fl[1]);
             }
         }
 
@@ -327,6 +324,7 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
                 issue_loads(round, L + 2);
             }
             const double ezm = __ldg(p.ezm + jc), ezp = __ldg(p.ezp + jc);
+            asm volatile("" : "+d"(fi0)); // keep the per-row geometry out of registers across lines
             wait_slot(L + 1);
 
             // ---- line j of the current level: the two r neighbours of the thread's 8 nodes
@@ -341,9 +339,10 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
             if (!edgeR) hr = lds64(sc + hro);
             else if (CL > 1 && crank < CL - 1) hr = lds64(halo_a + (q & 3u) * 32u + 16u);
 
-            // ---- level 1: assemble (13)/(15) and sweep (12) the thread's 8 rows
+            // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 8 rows
             double al[8], be[8], gm[8];
             {
+                if (anysp && ks >= 0) cA = load_coef<DEGK>(lay[cd & 0xffu], p.inv_tau, qa);
                 SweepState st;
                 st.om = 1.0; st.be = 0.0; st.gm = 1.0;
                 double2 tl = lds128(sc + co[0]);
@@ -359,9 +358,25 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const int k = 2 * qq + e;
+                        const double T = e ? tl.y : tl.x;
+                        // interface node (18)-(20) P:L176-192: lam*_A, lam*_B at T_{i*,j};
+                        // from here on the chunk belongs to layer B
+                        const bool isif = anysp && (k == ks);
+                        double lamA = 0.0;
+                        if (isif) {
+                            lamA = lam_eval<DEGK>(cA, true, T + T);
+                            cA = load_coef<DEGK>(lay[(cd >> 8) & 0xffu], p.inv_tau, qa);
+                        }
                         double cfR, w, f;
-                        regular_row<DEGK>(cA, anysq, e ? tl.y : tl.x, e ? tn.x : tl.y, e ? tu.y : tu.x, e ? fd.y : fd.x,
+                        regular_row<DEGK>(cA, anysq, T, e ? tn.x : tl.y, e ? tu.y : tu.x, e ? fd.y : fd.x,
                                           fi0 + (double)k, g0, ezp, ezm, cfR, w, f, fu[e]);
+                        const double cfNext = cfR; // face i + 1/2 as the next regular row sees it
+                        if (isif) {
+                            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
+                            st.cfL = lamA;
+                            cfR = lam_eval<DEGK>(cA, true, T + T);
+                            w = 0.0; f = 0.0;
+                        }
                         if (k == 7) { // r_out boundary row (15),(17) P:L158-174
                             st.cfL = last ? p.rout_a : st.cfL;
                             cfR = last ? 0.0 : cfR;
@@ -369,6 +384,7 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
                             f = last ? p.rout_f : f;
                         }
                         sweep_row(st, cfR, w, f, al[k]);
+                        if (isif) st.cfL = cfNext;
                         if (k == 0) { // r_in boundary row (15),(16) P:L158-169
                             al[0] = first ? 1.0 - p.rin_om : al[0];
                             st.om = first ? p.rin_om : st.om;
@@ -379,57 +395,6 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
                     }
                     sts128(fw + co[qq], fu[0], fu[1]);
                     tl = tn;
-                }
-            }
-
-            // ---- fix-up: the chunk holds an interface node (18)-(20) P:L176-192 at row ks;
-            //      rows above it belong to layer B.  Redo rows ks..7 (rare, one lane per interface).
-            if (__builtin_expect(ks >= 0, 0)) {
-                const PLayer *LA = lay + (cd & 0xffu), *LB = lay + ((cd >> 8) & 0xffu);
-                const double qsB = LB->heater ? qa * LB->src : 0.0;
-                SweepState s2;
-                s2.om = 1.0; s2.be = 0.0; s2.gm = 1.0; s2.cfL = 0.0;
-#pragma unroll
-                for (int k = 0; k < 7; ++k)
-                    if (k == ks - 1) { s2.om = 1.0 - al[k]; s2.be = be[k]; s2.gm = gm[k]; }
-                double Tp = hl;
-#pragma unroll
-                for (int qq = 0; qq < 4; ++qq) {
-                    const double2 tc = lds128(sc + co[qq]);
-                    const double tnx = (qq < 3) ? lds64(sc + co[qq < 3 ? qq + 1 : 3]) : hr;
-                    const double2 tu = lds128(su + co[qq]);
-                    const double2 fd = lds128(fr + co[qq]);
-                    double2 fu = lds128(fw + co[qq]);
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int k = 2 * qq + e;
-                        const double Tl_ = e ? tc.x : Tp, T_ = e ? tc.y : tc.x, Tr_ = e ? tnx : tc.y;
-                        const double Tu_ = e ? tu.y : tu.x, fD_ = e ? fd.y : fd.x;
-                        if (k < ks) continue;
-                        double cfR, w, f;
-                        if (k == ks) {
-                            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0,
-                            // lam* at T_{i*,j}; new level (reading G7)
-                            s2.cfL = lam_smem<DEGK>(LA, T_ + T_);
-                            cfR = lam_smem<DEGK>(LB, T_ + T_);
-                            w = 0.0; f = 0.0;
-                        } else {
-                            const double fi = fi0 + (double)k;
-                            s2.cfL = lam_smem<DEGK>(LB, Tl_ + T_) * fma(g0, fi, -0.5 * g0);
-                            cfR = lam_smem<DEGK>(LB, T_ + Tr_) * fma(g0, fi, 0.5 * g0);
-                            w = cap_smem(LB, T_, p.inv_tau) * fi;
-                            const double fuk = lam_smem<DEGK>(LB, T_ + Tu_) * (Tu_ - T_);
-                            double lz = fma(ezp, fuk, qsB);
-                            lz = fma(-ezm, fD_, lz);
-                            f = fma(w, T_, fi * lz);
-                            if (e) fu.y = fuk; else fu.x = fuk;
-                            if (k == 7 && last) { s2.cfL = p.rout_a; cfR = 0.0; w = p.rout_w; f = p.rout_f; }
-                        }
-                        sweep_row(s2, cfR, w, f, al[k]);
-                        be[k] = s2.be; gm[k] = s2.gm;
-                    }
-                    sts128(fw + co[qq], fu.x, fu.y);
-                    Tp = tc.y;
                 }
             }
 
