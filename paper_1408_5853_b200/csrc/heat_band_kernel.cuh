@@ -36,6 +36,18 @@ __device__ __forceinline__ void bulk_load_16(uint32_t dst, const void *src, uint
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 16, [%2];"
                  ::"r"(dst), "l"(src), "r"(bar) : "memory");
 }
+__device__ __forceinline__ double2 ld_cluster_v2(uint32_t a)
+{
+    double2 v;
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+// 16-byte store into the shared memory of a CTA of the cluster, completing on that CTA's mbarrier
+__device__ __forceinline__ void st_async_v2(uint32_t remote_addr, double x, double y, uint32_t remote_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 ::"r"(remote_addr), "d"(x), "d"(y), "r"(remote_bar) : "memory");
+}
 __device__ __forceinline__ void tma_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 
 // reciprocal: MUFU.RCP64H seed (>= 20 bits) + one cubic step e -> e^3: ~2^-60 before rounding
@@ -143,6 +155,99 @@ __device__ __forceinline__ void regular_row(const BCoef<DEGK> &c, bool anysq, do
     f = fma(w, T, fi * lz);
 }
 
+// Arguments of the 8-row sweep of one thread (all in registers after inlining).
+template <int DEGK>
+struct SweepArgs {
+    uint32_t sc, su, fr, fw; // shared addresses: line j, line j+1, lower flux (read), upper flux (write)
+    double hl, hr;           // r neighbours of the chunk at line j
+    double fi0, g0, ezp, ezm, inv_tau, qa;
+    uint32_t cd;
+    int ks;
+    bool first, last;
+    double rin_om, rin_be, rout_a, rout_w, rout_f;
+    const PLayer *lay;
+};
+
+// Level 1 for one thread: rows (13) P:L140-145 assembled and pushed through the sweep (12); with
+// SP also the interface row (18)-(20) P:L176-192 at row ks (the chunk's laws switch to layer B
+// there) and the r-boundary rows (15)-(17) P:L158-174 at rows 0 / 7 of the first / last chunk.
+template <int DEGK, bool SQ, bool SP>
+__device__ __forceinline__ void sweep8(const SweepArgs<DEGK> &A, const uint32_t (&co)[4], BCoef<DEGK> &cA,
+                                       double (&al)[8], double (&be)[8], double (&gm)[8])
+{
+    if (SP && A.ks >= 0) cA = load_coef<DEGK>(A.lay[A.cd & 0xffu], A.inv_tau, A.qa);
+    SweepState st;
+    st.om = 1.0; st.be = 0.0; st.gm = 1.0;
+    double2 tl = lds128(A.sc + co[0]);
+    st.cfL = lam_eval<DEGK>(cA, SQ, A.hl + tl.x) * fma(A.g0, A.fi0, -0.5 * A.g0); // face i0 - 1/2
+#pragma unroll
+    for (int qq = 0; qq < 4; ++qq) {
+        double2 tn;
+        if (qq < 3) tn = lds128(A.sc + co[qq < 3 ? qq + 1 : 3]);
+        else tn = make_double2(A.hr, A.hr);
+        const double2 tu = lds128(A.su + co[qq]);
+        const double2 fd = lds128(A.fr + co[qq]);
+        double fu[2];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int k = 2 * qq + e;
+            const double T = e ? tl.y : tl.x;
+            // interface node: lam*_A, lam*_B at T_{i*,j}; from here on the chunk is layer B
+            const bool isif = SP && (k == A.ks);
+            double lamA = 0.0;
+            if (SP && isif) {
+                lamA = lam_eval<DEGK>(cA, true, T + T);
+                cA = load_coef<DEGK>(A.lay[(A.cd >> 8) & 0xffu], A.inv_tau, A.qa);
+            }
+            double cfR, w, f;
+            regular_row<DEGK>(cA, SQ, T, e ? tn.x : tl.y, e ? tu.y : tu.x, e ? fd.y : fd.x,
+                              A.fi0 + (double)k, A.g0, A.ezp, A.ezm, cfR, w, f, fu[e]);
+            const double cfNext = cfR; // face i + 1/2 as the next regular row sees it
+            if (SP && isif) {
+                // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
+                st.cfL = lamA;
+                cfR = lam_eval<DEGK>(cA, true, T + T);
+                w = 0.0; f = 0.0;
+            }
+            if (SP && k == 7) { // r_out boundary row (15),(17) P:L158-174
+                st.cfL = A.last ? A.rout_a : st.cfL;
+                cfR = A.last ? 0.0 : cfR;
+                w = A.last ? A.rout_w : w;
+                f = A.last ? A.rout_f : f;
+            }
+            sweep_row(st, cfR, w, f, al[k]);
+            if (SP && isif) st.cfL = cfNext;
+            if (SP && k == 0) { // r_in boundary row (15),(16) P:L158-169
+                al[0] = A.first ? 1.0 - A.rin_om : al[0];
+                st.om = A.first ? A.rin_om : st.om;
+                st.be = A.first ? A.rin_be : st.be;
+                st.gm = A.first ? 0.0 : st.gm;
+            }
+            be[k] = st.be; gm[k] = st.gm;
+        }
+        sts128(A.fw + co[qq], fu[0], fu[1]);
+        tl = tn;
+    }
+}
+
+// PCR over lanes 0..30 of a warp; lane 31 (the separator) runs along and produces values nobody
+// reads.  On exit row i reads a_i*U + x_i + c_i*V = d_i (U left of lane 0, V = lane 31's unknown).
+__device__ __forceinline__ Row3 pcr_lanes_0_30(Row3 row, int lane)
+{
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+        Row3 L, R;
+        L.a = __shfl_up_sync(0xffffffffu, row.a, s);
+        L.c = __shfl_up_sync(0xffffffffu, row.c, s);
+        L.d = __shfl_up_sync(0xffffffffu, row.d, s);
+        R.a = __shfl_down_sync(0xffffffffu, row.a, s);
+        R.c = __shfl_down_sync(0xffffffffu, row.c, s);
+        R.d = __shfl_down_sync(0xffffffffu, row.d, s);
+        row = pcr_combine(row, L, lane >= s, R, lane + s <= 30);
+    }
+    return row;
+}
+
 // G  = threads of this CTA that work on one line (64, 128 or 256); CTA = 256 threads.
 // CL = cluster size; CL > 1 needs G == 256: the line has 256*CL threads, rank c owns nodes
 //      [2048c, 2048c + 2048).
@@ -152,6 +257,7 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
 {
     using Cfg = BandCfg<G, CL>;
     constexpr int SLOT = Cfg::SLOT;
+    constexpr uint32_t NSLOT = Cfg::NSLOT;
     constexpr int LPB = Cfg::LPB;
     constexpr int WG = Cfg::WG;
     constexpr int NSEP = Cfg::NSEP;
@@ -193,7 +299,7 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
         reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.players)[q];
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < 4; ++s) mbar_init(mbar_a + 8u * s, 1);
+        for (int s = 0; s < Cfg::NSLOT + 2; ++s) mbar_init(mbar_a + 8u * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -205,12 +311,14 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
     double fi0 = (double)i0;
     uint32_t qbase = 0;   // load sequence number of line offset -1 of this round
     uint32_t pubpar = 0;  // parity of the separator exchange buffer
+    uint32_t lcount = 0;  // lines done (phase of the exchange barriers)
 
     // line offset L (-1 .. BL) of this CTA's bands -> TMA loads into slot (qbase+L+1)&3
     auto issue_loads = [&](int round, int L) {
         const uint32_t q = qbase + (uint32_t)(L + 1);
-        const uint32_t slot = sbase + (q & 3u) * (uint32_t)SLOT;
-        const uint32_t bar = mbar_a + 8u * (q & 3u);
+        const uint32_t sl = q % NSLOT;
+        const uint32_t slot = sbase + sl * (uint32_t)SLOT;
+        const uint32_t bar = mbar_a + 8u * sl;
         uint32_t bytes = 0;
         int R[LPB];
 #pragma unroll
@@ -234,18 +342,18 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
             if (R[g] >= 0) tma_load_2d(slot + (uint32_t)(g * G * 64), &p.tm_ld, 0, R[g], bar);
         if (CL > 1 && R[0] >= 0) {
             const double *row0 = p.Told + (size_t)R[0] * 16;
-            if (crank > 0) bulk_load_16(halo_a + (q & 3u) * 32u, row0 - 2, bar);
-            if (crank < CL - 1) bulk_load_16(halo_a + (q & 3u) * 32u + 16u, row0 + (size_t)(G / 2) * 16, bar);
+            if (crank > 0) bulk_load_16(halo_a + sl * 32u, row0 - 2, bar);
+            if (crank < CL - 1) bulk_load_16(halo_a + sl * 32u + 16u, row0 + (size_t)(G / 2) * 16, bar);
         }
     };
     auto wait_slot = [&](int L) {
         const uint32_t q = qbase + (uint32_t)(L + 1);
-        while (!mbar_try_wait(mbar_a + 8u * (q & 3u), (q >> 2) & 1u)) {}
+        while (!mbar_try_wait(mbar_a + 8u * (q % NSLOT), (q / NSLOT) & 1u)) {}
     };
     // line offset L of this CTA's bands -> TMA stores of the new level from its slot
     auto issue_stores = [&](int round, int L) {
         const uint32_t q = qbase + (uint32_t)(L + 1);
-        const uint32_t slot = sbase + (q & 3u) * (uint32_t)SLOT;
+        const uint32_t slot = sbase + (q % NSLOT) * (uint32_t)SLOT;
 #pragma unroll
         for (int g = 0; g < LPB; ++g) {
             const int band = (round * nclusters + cluster_id) * LPB + g;
@@ -279,21 +387,19 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
         const int ks = (int)((cd >> 16) & 0xfu) - 1;
         const bool first = (cd & BD_FIRST) != 0, last = (cd & BD_LAST) != 0;
         // a chunk with an interface node switches to the laws of layer B behind it (warp-uniform flag)
-        const bool anysp = __any_sync(FULL, ks >= 0);
+        const bool anysp = __any_sync(FULL, ks >= 0 || first || last);
         const bool anysq = __any_sync(FULL, cA.sq || (ks >= 0 && lay[(cd >> 8) & 0xffu].sqrtk != 0));
 
         if (tid == 32) { // thread 32 issues every TMA load and store (bulk groups are per thread)
-            issue_loads(round, -1);
-            issue_loads(round, 0);
-            issue_loads(round, 1);
+            for (int Lp = -1; Lp <= min(2, BL); ++Lp) issue_loads(round, Lp);
         }
         wait_slot(-1);
         wait_slot(0);
 
         // ---- prologue: the flux through the faces between lines j0-1 and j0
         {
-            const uint32_t sd = sbase + ((qbase + 0u) & 3u) * (uint32_t)SLOT;
-            const uint32_t sc = sbase + ((qbase + 1u) & 3u) * (uint32_t)SLOT;
+            const uint32_t sd = sbase + ((qbase + 0u) % NSLOT) * (uint32_t)SLOT;
+            const uint32_t sc = sbase + ((qbase + 1u) % NSLOT) * (uint32_t)SLOT;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const double2 td = lds128(sd + co[q]);
@@ -312,17 +418,14 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
 
         for (int L = 0; L < BL; ++L) {
             const uint32_t q = qbase + (uint32_t)(L + 1);
-            const uint32_t sc = sbase + (q & 3u) * (uint32_t)SLOT;        // line j   (centre)
-            const uint32_t su = sbase + ((q + 1u) & 3u) * (uint32_t)SLOT; // line j+1 (up)
-            const uint32_t fr = sbase + Cfg::OFF_FLUX + (uint32_t)(L & 1) * (uint32_t)SLOT;       // fD
-            const uint32_t fw = sbase + Cfg::OFF_FLUX + (uint32_t)((L & 1) ^ 1) * (uint32_t)SLOT; // fU
+            const uint32_t qs = q % NSLOT, qu = (q + 1u) % NSLOT;
+            const uint32_t sc = sbase + qs * (uint32_t)SLOT; // line j   (centre)
+            const uint32_t su = sbase + qu * (uint32_t)SLOT; // line j+1 (up)
+            const uint32_t fr = sbase + Cfg::OFF_FLUX;       // lower flux fD, replaced in place by fU
+            const uint32_t fw = fr;
             const int j = j0 + L;
             const bool line_live = live && (j < j1);
             const int jc = min(j, nz - 2);
-            if (tid == 32 && L + 2 <= BL) {
-                tma_wait_read0(); // the store that last used the prefetch slot has read it
-                issue_loads(round, L + 2);
-            }
             const double ezm = __ldg(p.ezm + jc), ezp = __ldg(p.ezp + jc);
             asm volatile("" : "+d"(fi0)); // keep the per-row geometry out of registers across lines
             wait_slot(L + 1);
@@ -335,66 +438,26 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
                 hl = v0.x; hr = v3.y;
             }
             if (!edgeL) hl = lds64(sc + hlo);
-            else if (CL > 1 && crank > 0) hl = lds64(halo_a + (q & 3u) * 32u + 8u);
+            else if (CL > 1 && crank > 0) hl = lds64(halo_a + qs * 32u + 8u);
             if (!edgeR) hr = lds64(sc + hro);
-            else if (CL > 1 && crank < CL - 1) hr = lds64(halo_a + (q & 3u) * 32u + 16u);
+            else if (CL > 1 && crank < CL - 1) hr = lds64(halo_a + qs * 32u + 16u);
 
-            // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 8 rows
+            // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 8 rows; the code path
+            //      is chosen per warp: SQ = some lane has a square-root law, SP = some lane holds an
+            //      interface node or an r-boundary row
             double al[8], be[8], gm[8];
             {
-                if (anysp && ks >= 0) cA = load_coef<DEGK>(lay[cd & 0xffu], p.inv_tau, qa);
-                SweepState st;
-                st.om = 1.0; st.be = 0.0; st.gm = 1.0;
-                double2 tl = lds128(sc + co[0]);
-                st.cfL = lam_eval<DEGK>(cA, anysq, hl + tl.x) * fma(g0, fi0, -0.5 * g0); // face i0 - 1/2
-#pragma unroll
-                for (int qq = 0; qq < 4; ++qq) {
-                    double2 tn;
-                    if (qq < 3) tn = lds128(sc + co[qq < 3 ? qq + 1 : 3]);
-                    else tn = make_double2(hr, hr);
-                    const double2 tu = lds128(su + co[qq]);
-                    const double2 fd = lds128(fr + co[qq]);
-                    double fu[2];
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int k = 2 * qq + e;
-                        const double T = e ? tl.y : tl.x;
-                        // interface node (18)-(20) P:L176-192: lam*_A, lam*_B at T_{i*,j};
-                        // from here on the chunk belongs to layer B
-                        const bool isif = anysp && (k == ks);
-                        double lamA = 0.0;
-                        if (isif) {
-                            lamA = lam_eval<DEGK>(cA, true, T + T);
-                            cA = load_coef<DEGK>(lay[(cd >> 8) & 0xffu], p.inv_tau, qa);
-                        }
-                        double cfR, w, f;
-                        regular_row<DEGK>(cA, anysq, T, e ? tn.x : tl.y, e ? tu.y : tu.x, e ? fd.y : fd.x,
-                                          fi0 + (double)k, g0, ezp, ezm, cfR, w, f, fu[e]);
-                        const double cfNext = cfR; // face i + 1/2 as the next regular row sees it
-                        if (isif) {
-                            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
-                            st.cfL = lamA;
-                            cfR = lam_eval<DEGK>(cA, true, T + T);
-                            w = 0.0; f = 0.0;
-                        }
-                        if (k == 7) { // r_out boundary row (15),(17) P:L158-174
-                            st.cfL = last ? p.rout_a : st.cfL;
-                            cfR = last ? 0.0 : cfR;
-                            w = last ? p.rout_w : w;
-                            f = last ? p.rout_f : f;
-                        }
-                        sweep_row(st, cfR, w, f, al[k]);
-                        if (isif) st.cfL = cfNext;
-                        if (k == 0) { // r_in boundary row (15),(16) P:L158-169
-                            al[0] = first ? 1.0 - p.rin_om : al[0];
-                            st.om = first ? p.rin_om : st.om;
-                            st.be = first ? p.rin_be : st.be;
-                            st.gm = first ? 0.0 : st.gm;
-                        }
-                        be[k] = st.be; gm[k] = st.gm;
-                    }
-                    sts128(fw + co[qq], fu[0], fu[1]);
-                    tl = tn;
+                SweepArgs<DEGK> A;
+                A.sc = sc; A.su = su; A.fr = fr; A.fw = fw; A.hl = hl; A.hr = hr; A.fi0 = fi0; A.g0 = g0;
+                A.ezp = ezp; A.ezm = ezm; A.inv_tau = p.inv_tau; A.qa = qa; A.cd = cd; A.ks = ks;
+                A.first = first; A.last = last; A.rin_om = p.rin_om; A.rin_be = p.rin_be;
+                A.rout_a = p.rout_a; A.rout_w = p.rout_w; A.rout_f = p.rout_f; A.lay = lay;
+                if (!anysq) {
+                    if (!anysp) sweep8<DEGK, false, false>(A, co, cA, al, be, gm);
+                    else sweep8<DEGK, false, true>(A, co, cA, al, be, gm);
+                } else {
+                    if (!anysp) sweep8<DEGK, true, false>(A, co, cA, al, be, gm);
+                    else sweep8<DEGK, true, true>(A, co, cA, al, be, gm);
                 }
             }
 
@@ -420,43 +483,51 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
                 row.d = fma(al[7], Qn, be[7]) * r;
             }
             // ---- level 2: PCR over lanes 0..30; lane 31 is the warp's separator
-            const Row3 rp = pcr_segment<32>(row, lane, 0, 30);
+            const Row3 rp = pcr_lanes_0_30(row, lane);
             Row3 r30;
             r30.a = __shfl_sync(FULL, rp.a, 30);
             r30.c = __shfl_sync(FULL, rp.c, 30);
             r30.d = __shfl_sync(FULL, rp.d, 30);
-            {
-                const uint32_t slot = pub_a + (uint32_t)((pubpar * NSEP + gs) * Cfg::PUB) * 8u;
-                if (lane == 0 || lane == 31) {
-                    const uint32_t s6 = slot + (lane == 31 ? 48u : 0u);
-                    const double v0 = lane == 31 ? al[7] : P, v1 = lane == 31 ? be[7] : Q, v2 = lane == 31 ? gm[7] : S;
-                    const double v3 = lane == 31 ? r30.a : rp.a, v4 = lane == 31 ? r30.c : rp.c, v5 = lane == 31 ? r30.d : rp.d;
-                    if (CL > 1) {
+            // publish what the separator solve needs from this warp (12 doubles) to every CTA of the
+            // cluster: asynchronous DSMEM stores that complete on the receiver's mbarrier, so no
+            // cluster-wide barrier and no release fence are needed
+            const uint32_t pbar = sbase + Cfg::OFF_XBAR + 8u * pubpar;
+            if (lane == 0 || lane == 31) {
+                const uint32_t s6 = pub_a + (uint32_t)((pubpar * NSEP + gs) * Cfg::PUB) * 8u + (lane == 31 ? 48u : 0u);
+                const double v0 = lane == 31 ? al[7] : P, v1 = lane == 31 ? be[7] : Q, v2 = lane == 31 ? gm[7] : S;
+                const double v3 = lane == 31 ? r30.a : rp.a, v4 = lane == 31 ? r30.c : rp.c, v5 = lane == 31 ? r30.d : rp.d;
+                if (CL > 1) {
 #pragma unroll
-                        for (int rk = 0; rk < CL; ++rk) {
-                            const uint32_t ra = map_to_rank(s6, (uint32_t)rk);
-                            st_cluster_f64(ra, v0); st_cluster_f64(ra + 8, v1); st_cluster_f64(ra + 16, v2);
-                            st_cluster_f64(ra + 24, v3); st_cluster_f64(ra + 32, v4); st_cluster_f64(ra + 40, v5);
-                        }
-                    } else {
-                        sts64(s6, v0); sts64(s6 + 8, v1); sts64(s6 + 16, v2);
-                        sts64(s6 + 24, v3); sts64(s6 + 32, v4); sts64(s6 + 40, v5);
+                    for (int rk = 0; rk < CL; ++rk) {
+                        const uint32_t ra = map_to_rank(s6, (uint32_t)rk), rb = map_to_rank(pbar, (uint32_t)rk);
+                        st_async_v2(ra, v0, v1, rb);
+                        st_async_v2(ra + 16, v2, v3, rb);
+                        st_async_v2(ra + 32, v4, v5, rb);
                     }
+                } else {
+                    sts128(s6, v0, v1); sts128(s6 + 16, v2, v3); sts128(s6 + 32, v4, v5);
                 }
             }
-            if (CL > 1) { cluster_arrive(); cluster_wait(); } else __syncthreads();
+            if (CL == 1) __syncthreads();
             // ---- level 3: warp 0 builds every separator row and solves them (PCR per line)
             if (warp == 0) {
+                if (CL > 1) {
+                    if (lane == 0) mbar_expect_tx(pbar, (uint32_t)(NSEP * Cfg::PUB * 8));
+                    while (!mbar_try_wait(pbar, (lcount >> 1) & 1u)) {}
+                }
                 const bool in3 = lane < NSEP;
                 const int s = in3 ? lane : 0;
-                const double *D = pub + (pubpar * NSEP + s) * Cfg::PUB;
                 const bool has_next = ((s % WG) + 1 < WG);
-                const double *Dn = D + (has_next ? Cfg::PUB : 0);
-                const double sal = D[6], sbe = D[7], sgm = D[8];
-                Row3 l30; l30.a = D[9]; l30.c = D[10]; l30.d = D[11];
+                const int sn = has_next ? s + 1 : s;
+                const uint32_t Da = pub_a + (uint32_t)((pubpar * NSEP + s) * Cfg::PUB) * 8u;
+                const uint32_t Dn = pub_a + (uint32_t)((pubpar * NSEP + sn) * Cfg::PUB) * 8u;
+                const double2 d3 = lds128(Da + 48), d4 = lds128(Da + 64), d5 = lds128(Da + 80);
+                const double2 n0 = lds128(Dn), n1 = lds128(Dn + 16), n2 = lds128(Dn + 32);
+                const double sal = d3.x, sbe = d3.y, sgm = d4.x;
+                Row3 l30; l30.a = d4.y; l30.c = d5.x; l30.d = d5.y;
                 Row3 nx; nx.a = nx.c = nx.d = 0.0;
                 double Pw = 0.0, Qw = 0.0, Sw = 0.0;
-                if (has_next) { Pw = Dn[0]; Qw = Dn[1]; Sw = Dn[2]; nx.a = Dn[3]; nx.c = Dn[4]; nx.d = Dn[5]; }
+                if (has_next) { Pw = n0.x; Qw = n0.y; Sw = n1.x; nx.a = n1.y; nx.c = n2.x; nx.d = n2.y; }
                 Row3 me;
                 const double r = rcp_cubic(fma(-sal, Sw, 1.0));
                 me.a = -sgm * r;
@@ -465,11 +536,16 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
                 Row3 s3 = pcr_combine(me, l30, true, nx, has_next);
                 s3 = pcr_segment<WG>(s3, s % WG, 0, WG - 1);
                 if (in3) ysep[s] = s3.d;
-            } else if (tid == 32 && L > 0) {
-                issue_stores(round, L - 1); // every thread passed the barrier after writing line L-1
             }
             __syncthreads();
+            if (tid == 32) {
+                // every thread wrote line L-1 before this barrier: store it, then refill the slot of
+                // line L-2 (its store has read it) with line L+3
+                if (L > 0) issue_stores(round, L - 1);
+                if (L + 3 <= BL) { tma_wait_read1(); issue_loads(round, L + 3); }
+            }
             pubpar ^= 1u;
+            ++lcount;
             double y, u;
             {
                 const double Vs = ysep[gs];

@@ -55,12 +55,14 @@ struct BandCfg {
     static constexpr int NSEP = (NT / 32) * CL;
     static constexpr int SLOT = NT * 64;     // bytes of one staged line tile
     static constexpr int PUB = 12;
-    static constexpr int OFF_FLUX = 4 * SLOT;
+    static constexpr int NSLOT = 5;           // ring of staged lines: j-1 (store draining), j, j+1, j+2, j+3
+    static constexpr int OFF_FLUX = NSLOT * SLOT;
     static constexpr int OFF_HALO = 6 * SLOT;
-    static constexpr int OFF_PUB = OFF_HALO + 128;
+    static constexpr int OFF_PUB = OFF_HALO + 256;
     static constexpr int OFF_YSEP = OFF_PUB + 2 * NSEP * PUB * 8;
     static constexpr int OFF_MBAR = OFF_YSEP + NSEP * 8;
-    static constexpr int OFF_LAY = OFF_MBAR + 4 * 8;
+    static constexpr int OFF_XBAR = OFF_MBAR + NSLOT * 8; // separator-exchange barriers
+    static constexpr int OFF_LAY = OFF_XBAR + 2 * 8;
     static constexpr size_t smem_bytes(int nlayers) { return 1024 + (size_t)OFF_LAY + sizeof(PLayer) * (size_t)nlayers; }
 };
 
