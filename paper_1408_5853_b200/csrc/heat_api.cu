@@ -215,15 +215,11 @@ const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, s
     if (getenv("HEAT_VARIANT")) return nullptr;
     if (const char *e = getenv("HEAT_KERNEL"))
         if (strcmp(e, "line") == 0 || strcmp(e, "tma") == 0) return nullptr;
-    int G = 0, CL = 0;
-    switch (d->nr) {
-    case 512: G = 64; CL = 1; break;
-    case 1024: G = 128; CL = 1; break;
-    case 2048: G = 256; CL = 1; break;
-    case 4096: G = 256; CL = 2; break;
-    case 8192: G = 256; CL = 4; break;
-    default: return nullptr;
-    }
+    // threads per CTA: 256 (two CTAs per SM) or 128 (four per SM); a line takes nr/8 threads
+    int NT = 256;
+    if (const char *e = getenv("HEAT_BAND_NT")) NT = (atoi(e) == 128) ? 128 : 256;
+    if (d->nr != 512 && d->nr != 1024 && d->nr != 2048 && d->nr != 4096 && d->nr != 8192) return nullptr;
+    const int G = std::min(d->nr / 8, NT), CL = d->nr / 8 / G;
     if (d->face_mode != 0 || d->nz < 4) return nullptr;
     const int nr = d->nr, N = nr - 1;
     if (d->r[0] != 0.0) return nullptr;
@@ -264,7 +260,7 @@ const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, s
     if (players) *players = pl;
     if (cdesc) *cdesc = cd;
     for (int v = 0; v < k_nband_variants; ++v)
-        if (k_band_variants[v].G == G && k_band_variants[v].CL == CL && k_band_variants[v].DEGK == DEGK) return &k_band_variants[v];
+        if (k_band_variants[v].G == G && k_band_variants[v].CL == CL && k_band_variants[v].DEGK == DEGK && k_band_variants[v].NT == NT) return &k_band_variants[v];
     return nullptr;
 }
 
@@ -736,8 +732,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         {
             cudaLaunchConfig_t cfg;
             memset(&cfg, 0, sizeof cfg);
-            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * 2 * bv->CL), 1, 1);
-            cfg.blockDim = dim3(256, 1, 1);
+            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * (512 / bv->NT) * bv->CL), 1, 1);
+            cfg.blockDim = dim3((unsigned)bv->NT, 1, 1);
             cfg.dynamicSmemBytes = bsmem;
             cudaLaunchAttribute at[1];
             at[0].id = cudaLaunchAttributeClusterDimension;
@@ -749,7 +745,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / bv->CL);
         // bands: every group (256/G per CTA) walks BL consecutive lines of one batch member;
         // choose the band count per member that minimises rounds * (BL + prologue)
-        const int LPB = 256 / bv->G, Lz = nz - 2;
+        const int LPB = bv->NT / bv->G, Lz = nz - 2;
         const long long slots = (long long)max_clusters * LPB;
         long long best_cost = -1;
         int best_BL = Lz;
@@ -867,7 +863,7 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
             cudaLaunchConfig_t cfg;
             memset(&cfg, 0, sizeof cfg);
             cfg.gridDim = dim3((unsigned)c->grid, 1, 1);
-            cfg.blockDim = dim3(256, 1, 1);
+            cfg.blockDim = dim3((unsigned)c->bvar->NT, 1, 1);
             cfg.dynamicSmemBytes = c->smem;
             cfg.stream = st;
             cudaLaunchAttribute at[1];

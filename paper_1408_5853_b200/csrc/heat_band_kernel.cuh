@@ -248,21 +248,22 @@ __device__ __forceinline__ Row3 pcr_lanes_0_30(Row3 row, int lane)
     return row;
 }
 
-// G  = threads of this CTA that work on one line (64, 128 or 256); CTA = 256 threads.
-// CL = cluster size; CL > 1 needs G == 256: the line has 256*CL threads, rank c owns nodes
-//      [2048c, 2048c + 2048).
+// NT = threads per CTA (128 or 256).  G = threads of this CTA that work on one line (64 .. NT).
+// CL = cluster size; CL > 1 needs G == NT: the line has NT*CL threads, rank c owns nodes
+//      [8 NT c, 8 NT (c + 1)).
 // DEGK = degree of the lambda polynomials.
-template <int G, int CL, int DEGK>
-__global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant__ BParams p)
+template <int G, int CL, int DEGK, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) heat_band_kernel(const __grid_constant__ BParams p)
 {
-    using Cfg = BandCfg<G, CL>;
+    using Cfg = BandCfg<G, CL, NT>;
     constexpr int SLOT = Cfg::SLOT;
     constexpr uint32_t NSLOT = Cfg::NSLOT;
     constexpr int LPB = Cfg::LPB;
     constexpr int WG = Cfg::WG;
     constexpr int NSEP = Cfg::NSEP;
     constexpr uint32_t FULL = 0xffffffffu;
-    static_assert(CL == 1 || G == 256, "a cluster line needs whole CTAs");
+    static_assert(CL == 1 || G == NT, "a cluster line needs whole CTAs");
+    constexpr int NW = NT / 32;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     unsigned char *gbase = smem_raw + (sbase - smem_u32(smem_raw));
@@ -282,7 +283,7 @@ __global__ void __launch_bounds__(256, 2) heat_band_kernel(const __grid_constant
     const int t = crank * G + tg;       // thread within the line
     const int i0 = t * 8;
     const int wig = t >> 5;             // warp within the line
-    const int gs = crank * 8 + warp;    // this warp's separator slot
+    const int gs = crank * NW + warp;    // this warp's separator slot
     const int trow = tid >> 1, half = tid & 1, sw = trow & 7;
     // byte offsets inside a slot: own 16-byte chunks q = 0..3, and the two r neighbours
     const uint32_t rowo = (uint32_t)trow * 128u;

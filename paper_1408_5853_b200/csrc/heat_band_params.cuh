@@ -45,9 +45,9 @@ struct BParams {
     int bands_per_member, total_bands;
 };
 
-template <int G, int CL>
+template <int G, int CL, int NT_>
 struct BandCfg {
-    static constexpr int NT = 256;
+    static constexpr int NT = NT_;
     static constexpr int M = 8;
     static constexpr int LPB = NT / G;       // lines (bands) a CTA works on side by side
     static constexpr int GL = G * CL;        // threads per line

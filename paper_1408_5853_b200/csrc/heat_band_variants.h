@@ -10,7 +10,7 @@ namespace heat {
 
 typedef void (*band_kernel_fn)(const BParams);
 struct BandVariant {
-    int G, CL, DEGK;
+    int G, CL, DEGK, NT;
     band_kernel_fn fn;
     const char *name;
     size_t smem_fixed; // bytes without the layer table
