@@ -28,7 +28,9 @@ import numpy as np
 
 METRIC = "fp64 GCUPS (cell-updates/s) per FD time step"
 UNIT = "GCUPS"
-BYTES_PER_CELL = 16.0  # algorithmic: 8 B read of T^k + 8 B write of T^{k+1} (DESIGN.md "Roofline")
+BYTES_PER_CELL = 16.0  # algorithmic: 8 B read of T^k + 8 B write of T^{k+1} (DESIGN.md section 6)
+FP64_PER_CELL = 48.0   # fp64 thread-instructions per cell-update of the band kernel (ncu SASS counts)
+FP64_LANES = 148 * 64  # fp64 lanes of a B200 (64 per SM)
 
 
 def load_peaks():
@@ -42,11 +44,12 @@ def load_peaks():
 
 
 def load_traffic(kernel_name):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
-    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/roofline_traffic.txt, key=value lines); None if the capture is of another kernel."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.txt")
     if os.path.exists(p):
         try:
-            d = json.load(open(p))
+            d = dict(l.strip().split("=", 1) for l in open(p) if "=" in l)
             if d.get("kernel") == kernel_name:
                 return float(d["dram_bytes_per_launch"])
         except Exception:
@@ -268,6 +271,10 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "kernel": sim.kernel_name,
                      "bytes_per_launch": BYTES_PER_CELL * cells, "launch_ms": per_launch_ms},
+        "roofline_alu": {"bound": "alu", "achieved": achieved / BYTES_PER_CELL * FP64_PER_CELL, "unit": "G fp64 inst/s",
+                         "peak": FP64_LANES * (clk.summary()["sm_max_mhz"] or 1965.0) * 1e-3,
+                         "frac": achieved / BYTES_PER_CELL * FP64_PER_CELL / (FP64_LANES * (clk.summary()["sm_max_mhz"] or 1965.0) * 1e-3),
+                         "what": "co-limit: 48 fp64 instructions per cell-update on 148 x 64 lanes at the max SM clock"},
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * cells, "d2h_bytes_per_step": 8 * cells,
                 "steps": ke, "what": "heat_set_field(host pinned) + heat_step(1) + heat_get_field(host pinned) per step"},

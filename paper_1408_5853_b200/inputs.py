@@ -244,3 +244,52 @@ def random_spec(seed, nr=13, nz=11, nlayers=3, batch=1, laws="mixed", source=Tru
     s["probes"] = [(nr - 1, nz // 2), (1, 1)]
     s["probe_every"] = 2
     return s
+
+
+# ---------------------------------------------------------------- band-kernel edge cases
+
+def band_spec(seed, nr=512, nz=24, nlayers=4, batch=1, bcs=None, source=True, poly_laws=False,
+              nonuniform_z=True):
+    """Seeded problem on a uniform r grid starting at r = 0 (what the band kernel covers) with
+    interface nodes at every position of an 8-node chunk (first, last, middle), square-root,
+    power and polynomial laws, random initial field, optional source and non-uniform z."""
+    rng = np.random.Generator(np.random.PCG64(SEED + 1000 + int(seed)))
+    R = 2e-3
+    r = uniform_nodes(R, nr)
+    hz = rng.uniform(0.7, 1.3, size=nz - 1) if nonuniform_z else np.ones(nz - 1)
+    z = np.concatenate([[0.0], np.cumsum(hz)]) * (10.0 * R / (nr - 1))  # eta ~ 10 h as in BASELINE configs
+    layers = []
+    for m in range(nlayers):
+        if poly_laws:
+            k = poly([rng.uniform(1, 5), rng.uniform(0.1, 0.5), rng.uniform(1e-3, 5e-3), rng.uniform(1e-6, 1e-5),
+                      rng.uniform(1e-8, 1e-7) if m % 2 else 0.0])
+            cp = poly([rng.uniform(1, 5), rng.uniform(0.1, 0.5), rng.uniform(1e-3, 5e-3), rng.uniform(1e-5, 1e-4)])
+        else:
+            k = power(rng.uniform(1, 100), [1.0, 2.0, 1.5, 0.5, 3.0, 0.0][(m + seed) % 6])
+            cp = [power(rng.uniform(1, 10), 3.0), power(rng.uniform(1, 10), 2.0), const(rng.uniform(50, 200)),
+                  power(rng.uniform(1, 10), 1.0)][(m + seed) % 4]
+        layers.append(layer(k, cp, rng.uniform(2000, 9000), is_heater=(source and m == nlayers - 2)))
+    segs = []
+    for b in range(batch):
+        # one interface per chosen chunk, at chunk positions 0, 7 and a random one
+        chunks = sorted(rng.choice(np.arange(1, nr // 8 - 1), size=nlayers - 1, replace=False).tolist())
+        pos = [0, 7] + [int(rng.integers(1, 7)) for _ in range(nlayers)]
+        nodes = [8 * c + pos[(q + b) % len(pos)] for q, c in enumerate(chunks)]
+        # adjacent chunks could give adjacent interface nodes (8c+7, 8c+8): move the second one
+        for q in range(1, len(nodes)):
+            if nodes[q] - nodes[q - 1] < 2:
+                nodes[q] += 3
+        segs.append(seg_layers(nr, nodes))
+    s = _base(nr, nz, 1, 1, layers, np.stack(segs), batch)
+    s["r"], s["z"] = r, z
+    if bcs is not None:
+        s["r_in"], s["r_out"], s["z_lo"], s["z_hi"] = bcs
+    s["T_init"] = rng.uniform(5.0, 80.0, size=(batch, nz, nr))
+    s["T_lo"], s["T_hi"] = 4.2, 100.0
+    if source:
+        s["Q0"] = rng.uniform(1e8, 1e9, size=batch)
+        s["steps_per_period"], s["steps_on"] = 7, 3
+        s["transient_substeps"], s["transient_k"] = 5, 7.0
+    s["probes"] = [(nr - 1, nz // 2), (0, 1), (int(np.flatnonzero(np.diff(segs[0].astype(int)))[0]) + 1, nz - 2), (17, 0)]
+    s["probe_every"] = 2
+    return s

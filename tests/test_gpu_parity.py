@@ -106,6 +106,58 @@ def test_every_kernel_variant(bd, variant, monkeypatch):
         sim.close()
 
 
+BAND_CASES = [
+    # nr, nz, batch, poly laws, bcs, HEAT_BAND_NT
+    (512, 24, 3, False, None, 256),
+    (512, 9, 5, True, BC_SETS[1], 256),        # 5 bands on 4 groups per CTA: ragged last round
+    (1024, 21, 2, False, BC_SETS[2], 256),     # Dirichlet r boundaries
+    (2048, 19, 1, True, BC_SETS[3], 256),
+    (4096, 12, 1, False, None, 256),           # cluster of 2 CTAs per line
+    (8192, 7, 1, False, BC_SETS[1], 256),      # cluster of 4, Neumann z_lo
+    (512, 24, 3, False, None, 128),
+    (2048, 13, 2, True, BC_SETS[3], 128),      # cluster of 2 at 128 threads
+    (8192, 6, 1, False, None, 128),            # cluster of 8 (non-portable size)
+]
+
+
+@pytest.mark.parametrize("case", BAND_CASES, ids=lambda c: f"nr{c[0]}-nz{c[1]}-b{c[2]}-{'poly' if c[3] else 'pow'}-nt{c[5]}")
+def test_band_kernel_edge_cases(bd, case, monkeypatch):
+    """The band kernel (the one bench.py times) on seeded problems built to hit its special
+    paths: interface nodes at the first / last / middle row of a thread's 8-node chunk, square
+    root, power and degree-4 polynomial laws side by side in one warp, every BC kind, non-uniform
+    z, random initial field, source with sub-steps, probes on boundary / interface / Dirichlet
+    nodes, ragged band partition, clusters of 1, 2, 4 and 8 CTAs per line."""
+    nr, nz, batch, poly, bcs, nt = case
+    monkeypatch.setenv("HEAT_BAND_NT", str(nt))
+    s = I.band_spec(nr + nz, nr=nr, nz=nz, batch=batch, bcs=bcs, poly_laws=poly)
+    s = with_dt(bd, s, 0.8)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp" if nr * nz > 30000 else "double")
+    assert sim.kernel_name.startswith("band<") and sim.kernel_name.endswith(f"NT={nt}>"), sim.kernel_name
+    for n in (1, 6, 13):
+        sim.step(n)
+        orc.step(n)
+        compare(sim, orc)
+    pg, dropped = sim.probes()
+    po = orc.probes()
+    assert dropped == 0 and pg.shape == po.shape
+    assert np.max(np.abs(pg - po)) <= TOL
+    sim.close()
+
+
+def test_band_kernel_band_length_does_not_change_the_result(bd, monkeypatch):
+    """The partition of the lines into bands is a scheduling choice: the field is bitwise the
+    same for bands of 1, 3 and all lines."""
+    s = with_dt(bd, I.band_spec(7, nr=512, nz=20, batch=2), 0.8)
+    out = []
+    for bl in ("1", "3", "18"):
+        monkeypatch.setenv("HEAT_BAND_LINES", bl)
+        sim = bd.HeatSim(s)
+        sim.step(9)
+        out.append(sim.fields())
+        sim.close()
+    assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
+
+
 def test_schedule_table_is_bit_exact(bd):
     """(4) P:L79, (22) P:L212-217: the library's (tau_k, amp_k) equals the oracle's, bitwise."""
     s = I.random_spec(0, source=True)
