@@ -803,6 +803,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         bp.nr = nr; bp.nz = nz; bp.batch = d->batch; bp.nlayers = d->nlayers; bp.nprobes = d->nprobes;
         bp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
         bp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
+        bp.rank_rot = bv->CL / 2;
+        if (const char *er = getenv("HEAT_RANK_ROT")) bp.rank_rot = atoi(er);
         bp.rpl = nr / 16; bp.BL = best_BL; bp.bands_per_member = bpm; bp.total_bands = (int)bands;
     }
 

@@ -60,18 +60,17 @@ __device__ __forceinline__ double rcp_cubic(double x)
     return fma(y, t, y);
 }
 
-// square root for lambda ~ T^(p+1/2): MUFU.RSQ64H seed (>= 20 bits) + two coupled Newton steps
-// (g -> sqrt s, hy -> 1/(2 sqrt s)); relative error ~2^-52, no special cases (s > 0 here)
+// square root for lambda ~ T^(p+1/2): MUFU.RSQ64H seed y (>= 20 bits) + one cubic step on
+// sqrt s = s y (1 - h)^(-1/2), h = 1 - s y^2:  g = t + t h (1/2 + 3/8 h), t = s y; the truncation
+// error is 5/16 h^3 < 2^-61, so the result is within rounding of the exact root; s > 0 here
 __device__ __forceinline__ double sqrt_pos(double s)
 {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
-    double g = s * y, hy = 0.5 * y;
-    double r = fma(-hy, g, 0.5);
-    g = fma(g, r, g);
-    hy = fma(hy, r, hy);
-    r = fma(-hy, g, 0.5);
-    return fma(g, r, g);
+    const double t = s * y;
+    const double h = fma(-t, y, 1.0);
+    const double q = h * fma(0.375, h, 0.5);
+    return fma(t, q, t);
 }
 
 template <int DEGK>
@@ -277,7 +276,9 @@ __global__ void __launch_bounds__(NT, 512 / NT) heat_band_kernel(const __grid_co
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
-    const int crank = (CL > 1) ? (int)cluster_ctarank() : 0;
+    // rank of this CTA within the line: the hardware rank, rotated by p.rank_rot in odd clusters so
+    // that CTAs sharing an SM need not hold the same (possibly most expensive) part of the radius
+    const int crank = (CL > 1) ? (int)((cluster_ctarank() + (uint32_t)(((blockIdx.x / CL) & 1) ? p.rank_rot : 0)) % (uint32_t)CL) : 0;
     const int grp = tid / G;            // group (line) within the CTA
     const int tg = tid % G;             // thread within the CTA's part of the line
     const int t = crank * G + tg;       // thread within the line

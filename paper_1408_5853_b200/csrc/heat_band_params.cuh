@@ -43,6 +43,7 @@ struct BParams {
     int rpl;  // tensor rows (16 doubles) per line
     int BL;   // lines per band
     int bands_per_member, total_bands;
+    int rank_rot; // see heat_band_kernel: rotation of the cluster rank -> radius part map in odd clusters
 };
 
 template <int G, int CL, int NT_>
