@@ -172,21 +172,14 @@ def run_ours(args):
     import torch
     from paper_1408_5853_b200 import binding, build as B
     B.build()
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1408_5853_b200 import replicas as R
+    rank, local, world = R.rank_env()
     assert torch.cuda.is_available(), "bench.py needs a CUDA device; there is no CPU fallback"
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist_
-        dist = dist_
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dist = R.init("nccl", local, world)  # replicas only: no data-path collective
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
+        R.barrier(dist, torch.cuda.synchronize)
 
     spec = make_spec(args.config, binding.heat_stable_dt)
     cells = spec["nr"] * spec["nz"] * spec["batch"]
@@ -206,11 +199,8 @@ def run_ours(args):
         barrier()
     ms = e0.elapsed_time(e1)
     launches = sim.launch_count - l0
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * cells * K / (ms_max * 1e-3) / 1e9
+    ms_max = R.max_over_ranks(ms, dist, "cuda")
+    value = R.job_gcups(cells, K, ms_max * 1e-3, world)
     probes, _ = sim.probes()
     field_ok = bool(torch.isfinite(sim.field_device(0)).all().item())
 
@@ -239,10 +229,7 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * cells * ke / float(t.item()) / 1e9
+    e2e_value = R.job_gcups(cells, ke, R.max_over_ranks(e2e_s, dist, "cuda"), world)
 
     if rank != 0:
         if dist is not None:
