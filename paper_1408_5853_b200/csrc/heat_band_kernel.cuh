@@ -229,91 +229,6 @@ __device__ __forceinline__ void sweep8(const SweepArgs<DEGK> &A, const uint32_t 
     }
 }
 
-// One pair of rows (2 qq, 2 qq + 1) of one sweep chain: the body of sweep8's loop, with the chain's
-// own law coefficients c and sweep state st.  tl = (T_2qq, T_2qq+1), tn.x = T_2qq+2.
-template <int DEGK, bool SQ, bool SP>
-__device__ __forceinline__ void pair_rows(const SweepArgs<DEGK> &A, BCoef<DEGK> &c, SweepState &st, int qq, double2 tl,
-                                          double2 tn, double2 tu, double2 fd, double (&fu)[2], double (&al)[8],
-                                          double (&be)[8], double (&gm)[8])
-{
-#pragma unroll
-    for (int e = 0; e < 2; ++e) {
-        const int k = 2 * qq + e;
-        const double T = e ? tl.y : tl.x;
-        const bool isif = SP && (k == A.ks);
-        double lamA = 0.0;
-        if (SP && isif) { // interface node: lam*_A, lam*_B at T_{i*,j}; then the chunk is layer B
-            lamA = lam_eval<DEGK>(c, true, T + T);
-            c = load_coef<DEGK>(A.lay[(A.cd >> 8) & 0xffu], A.inv_tau, A.qa);
-        }
-        double cfR, w, f;
-        regular_row<DEGK>(c, SQ, T, e ? tn.x : tl.y, e ? tu.y : tu.x, e ? fd.y : fd.x, A.fi0 + (double)k, A.g0,
-                          A.ezp, A.ezm, cfR, w, f, fu[e]);
-        const double cfNext = cfR;
-        if (SP && isif) { // (18) times h (new level, G7)
-            st.cfL = lamA;
-            cfR = lam_eval<DEGK>(c, true, T + T);
-            w = 0.0; f = 0.0;
-        }
-        if (SP && k == 7) { // r_out boundary row (15),(17) P:L158-174
-            st.cfL = A.last ? A.rout_a : st.cfL;
-            cfR = A.last ? 0.0 : cfR;
-            w = A.last ? A.rout_w : w;
-            f = A.last ? A.rout_f : f;
-        }
-        sweep_row(st, cfR, w, f, al[k]);
-        if (SP && isif) st.cfL = cfNext;
-        if (SP && k == 0) { // r_in boundary row (15),(16) P:L158-169
-            al[0] = A.first ? 1.0 - A.rin_om : al[0];
-            st.om = A.first ? A.rin_om : st.om;
-            st.be = A.first ? A.rin_be : st.be;
-            st.gm = A.first ? 0.0 : st.gm;
-        }
-        be[k] = st.be; gm[k] = st.gm;
-    }
-}
-
-// Level 1 as TWO independent sweep chains per thread (instruction-level parallelism 2): chain A =
-// rows 0..3 with the left unknown u (last node of the thread to the left), chain B = rows 4..7
-// with the left unknown x_3.  On exit  x_k = al_k x_{k+1} + be_k + gm_k u   (k <= 3)  and
-// x_k = al_k x_{k+1} + be_k + gm_k x_3  (k >= 4).  The caller eliminates x_3.
-template <int DEGK, bool SQ, bool SP>
-__device__ __forceinline__ void sweep8x2(const SweepArgs<DEGK> &A, const uint32_t (&co)[4], BCoef<DEGK> &cA,
-                                         double (&al)[8], double (&be)[8], double (&gm)[8])
-{
-    if (SP && A.ks >= 0) cA = load_coef<DEGK>(A.lay[A.cd & 0xffu], A.inv_tau, A.qa);
-    BCoef<DEGK> cB = cA; // laws of rows 4..7: layer B from the start if the interface node is in rows 0..3
-    if (SP && A.ks >= 0 && A.ks < 4) cB = load_coef<DEGK>(A.lay[(A.cd >> 8) & 0xffu], A.inv_tau, A.qa);
-    const double2 t01 = lds128(A.sc + co[0]);
-    const double2 t45 = lds128(A.sc + co[2]);
-    const double2 t23 = lds128(A.sc + co[1]);
-    SweepState sa, sb;
-    sa.om = 1.0; sa.be = 0.0; sa.gm = 1.0;
-    sb.om = 1.0; sb.be = 0.0; sb.gm = 1.0;
-    sa.cfL = lam_eval<DEGK>(cA, SQ, A.hl + t01.x) * fma(A.g0, A.fi0, -0.5 * A.g0); // face i0 - 1/2
-    // face i0 + 3 1/2 as row 4 sees it: the law of segment (3, 4)
-    sb.cfL = lam_eval<DEGK>((SP && A.ks == 3) ? cB : ((SP && A.ks >= 0 && A.ks < 3) ? cB : cA), SQ, t23.y + t45.x) *
-             fma(A.g0, A.fi0, 3.5 * A.g0);
-    double fu[2];
-    {
-        const double2 tuA = lds128(A.su + co[0]), fdA = lds128(A.fr + co[0]);
-        const double2 tuB = lds128(A.su + co[2]), fdB = lds128(A.fr + co[2]);
-        pair_rows<DEGK, SQ, SP>(A, cA, sa, 0, t01, t23, tuA, fdA, fu, al, be, gm);
-        sts128(A.fw + co[0], fu[0], fu[1]);
-        pair_rows<DEGK, SQ, SP>(A, cB, sb, 2, t45, lds128(A.sc + co[3]), tuB, fdB, fu, al, be, gm);
-        sts128(A.fw + co[2], fu[0], fu[1]);
-    }
-    {
-        const double2 tuA = lds128(A.su + co[1]), fdA = lds128(A.fr + co[1]);
-        const double2 tuB = lds128(A.su + co[3]), fdB = lds128(A.fr + co[3]);
-        pair_rows<DEGK, SQ, SP>(A, cA, sa, 1, t23, t45, tuA, fdA, fu, al, be, gm);
-        sts128(A.fw + co[1], fu[0], fu[1]);
-        pair_rows<DEGK, SQ, SP>(A, cB, sb, 3, lds128(A.sc + co[3]), make_double2(A.hr, A.hr), tuB, fdB, fu, al, be, gm);
-        sts128(A.fw + co[3], fu[0], fu[1]);
-    }
-    if (SP) cA = cB; // as after sweep8: the coefficients of the chunk's last row
-}
-
 // PCR over lanes 0..30 of a warp; lane 31 (the separator) runs along and produces values nobody
 // reads.  On exit row i reads a_i*U + x_i + c_i*V = d_i (U left of lane 0, V = lane 31's unknown).
 __device__ __forceinline__ Row3 pcr_lanes_0_30(Row3 row, int lane)
