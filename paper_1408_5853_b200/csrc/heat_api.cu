@@ -366,6 +366,7 @@ struct heat_ctx {
     const Variant *var;
     const TmaVariant *tvar; // non-NULL: heat_step launches the TMA kernel
     const BandVariant *bvar; // non-NULL: heat_step launches the band kernel
+    int pdl;                 // band kernel: launch with programmatic stream serialization
     CUtensorMap btm_ld[2], btm_st[2];
     BParams bp;
     CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
@@ -489,6 +490,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     std::vector<uint32_t> bdesc;
     const BandVariant *bv = plan_band(d, &players, &bdesc);
     c->var = v; c->tvar = tv; c->bvar = bv; c->lay = L; c->ws = (char *)workspace;
+    // measured: 10.4 -> 8.7 us per step on 512 x 512, 36.9 -> 34.7 on 2048 x 2048; with clusters (nr >= 4096)
+    // the piecemeal placement of the next step's clusters costs 11 %, so it stays off there
+    c->pdl = (bv && bv->CL == 1) ? 1 : 0;
+    if (const char *ep = getenv("HEAT_PDL")) c->pdl = atoi(ep) != 0;
     c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
     c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
@@ -868,10 +873,14 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
             cfg.blockDim = dim3((unsigned)c->bvar->NT, 1, 1);
             cfg.dynamicSmemBytes = c->smem;
             cfg.stream = st;
-            cudaLaunchAttribute at[1];
+            cudaLaunchAttribute at[2];
             at[0].id = cudaLaunchAttributeClusterDimension;
             at[0].val.clusterDim.x = (unsigned)c->bvar->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-            cfg.attrs = at; cfg.numAttrs = 1;
+            // programmatic dependent launch: step k+1 may start its prologue while step k drains; it
+            // waits (griddepcontrol.wait) for step k to complete before it touches the field
+            at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            at[1].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = at; cfg.numAttrs = c->pdl ? 2 : 1;
             CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->bvar->fn, bp));
         } else if (c->tvar) {
             const int q = (c->cur == c->field_a) ? 0 : 1;

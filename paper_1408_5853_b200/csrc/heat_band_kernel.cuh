@@ -306,6 +306,11 @@ __global__ void __launch_bounds__(NT, 512 / NT) heat_band_kernel(const __grid_co
     }
     __syncthreads();
     if (CL > 1) { cluster_arrive(); cluster_wait(); }
+    // Programmatic dependent launch: everything above (shared-memory carve-up, barrier init, law
+    // table) overlaps the tail of the previous time step; the field is touched only from here on.
+    // The next step's CTAs may be scheduled as soon as this grid leaves room for them.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     const int nr = p.nr, nz = p.nz, BL = p.BL, bpm = p.bands_per_member;
     const int cluster_id = blockIdx.x / CL, nclusters = gridDim.x / CL;
