@@ -244,6 +244,12 @@ def run_ours(args):
     if world == 1 and not args.no_cpu_baseline:
         v, cores, desc, _ = oracle_sample(args.config, budget_s=12.0)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        # second reported baseline: the same oracle, OpenMP over the lines j (bitwise the same result)
+        try:
+            v2, cores2, desc2, _ = oracle_sample(args.config, budget_s=6.0, variant="omp")
+            cpu["omp"] = {"value": v2, "unit": UNIT, "cores": cores2, "sample": desc2}
+        except Exception as ex:  # the OpenMP build is optional
+            cpu["omp"] = {"unavailable": str(ex)[:120]}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
