@@ -158,6 +158,31 @@ def test_band_kernel_band_length_does_not_change_the_result(bd, monkeypatch):
     assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
 
 
+@pytest.mark.parametrize("nr", [128, 256, 512, 1024, 2048, 4096, 8192])
+@pytest.mark.parametrize("face_mode", [0, 1])
+def test_tma_kernel_variants(bd, nr, face_mode, monkeypatch):
+    """The TMA line kernel (the general fast path: any law kind, both face modes; heat_create
+    picks it when the band kernel does not cover the descriptor) on every line length it is
+    instantiated for, on the band kernel's edge-case problems."""
+    monkeypatch.setenv("HEAT_KERNEL", "tma")
+    nz = 9 if nr >= 2048 else 14
+    s = I.band_spec(3 * nr + face_mode, nr=nr, nz=nz, batch=2 if nr <= 1024 else 1, poly_laws=(nr // 128) % 2 == 1,
+                    bcs=BC_SETS[(nr // 128) % 4])
+    s["face_mode"] = face_mode
+    # the mean of two lambdas (face_mode 1) on a random field of 5..80 K exceeds lambda at the mean
+    # temperature by far: keep the explicit part well inside its stability range
+    s = with_dt(bd, s, 0.8 if face_mode == 0 else 0.25)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp" if nr * nz > 30000 else "double")
+    assert sim.kernel_name.startswith("tma<"), sim.kernel_name
+    for n in (1, 7, 12):
+        sim.step(n)
+        orc.step(n)
+        compare(sim, orc)
+    pg, dropped = sim.probes()
+    assert dropped == 0 and np.max(np.abs(pg - orc.probes())) <= TOL
+    sim.close()
+
+
 def test_schedule_table_is_bit_exact(bd):
     """(4) P:L79, (22) P:L212-217: the library's (tau_k, amp_k) equals the oracle's, bitwise."""
     s = I.random_spec(0, source=True)
