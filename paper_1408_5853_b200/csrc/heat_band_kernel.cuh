@@ -50,16 +50,6 @@ __device__ __forceinline__ void st_async_v2(uint32_t remote_addr, double x, doub
 }
 __device__ __forceinline__ void tma_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 
-// reciprocal: MUFU.RCP64H seed (>= 20 bits) + one cubic step e -> e^3: ~2^-60 before rounding
-__device__ __forceinline__ double rcp_cubic(double x)
-{
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-x, y, 1.0);
-    const double t = fma(e, e, e);
-    return fma(y, t, y);
-}
-
 // square root for lambda ~ T^(p+1/2): MUFU.RSQ64H seed y (>= 20 bits) + one cubic step on
 // sqrt s = s y (1 - h)^(-1/2), h = 1 - s y^2:  g = t + t h (1/2 + 3/8 h), t = s y; the truncation
 // error is 5/16 h^3 < 2^-61, so the result is within rounding of the exact root; s > 0 here

@@ -57,6 +57,16 @@ __device__ __forceinline__ double rcp_nr(double x)
     return y;
 }
 
+// reciprocal: MUFU.RCP64H seed (>= 20 bits) + one cubic step e -> e^3: ~2^-60 before rounding
+__device__ __forceinline__ double rcp_cubic(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
+}
+
 __device__ __forceinline__ double law_at(const DLaw &L, double T)
 {
     switch (L.kind) {

@@ -31,7 +31,7 @@ __device__ __forceinline__ Row3 pcr_combine(const Row3 &me, const Row3 &L, bool 
     const double ar = vr ? R.a : 0.0, dr = vr ? R.d : 0.0;
     double den = fma(-me.a, cl, 1.0);
     den = fma(-me.c, ar, den);
-    const double r = rcp_nr(den);
+    const double r = rcp_cubic(den);
     double d = fma(-me.a, dl, me.d);
     d = fma(-me.c, dr, d);
     Row3 o;
