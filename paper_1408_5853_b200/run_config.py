@@ -4,7 +4,8 @@ trace (the surface-temperature deliverable of configs 2-4).
     python -m paper_1408_5853_b200.run_config --config 2 --out gpurun_out/config2 [--steps N] [--every 10000]
 
 Writes <out>_summary.txt (wall time, throughput, per-period extrema of the first probe of batch
-member 0) and <out>_trace.csv (every `--every`-th probe record).  Only the C-ABI library is
+member 0), <out>_trace.csv (every `--every`-th probe record of member 0) and, for a batch,
+<out>_members.csv (one row per member: its parameters and the maximum / final probe value).  Only the C-ABI library is
 used (heat_create / heat_step / heat_probe / heat_get_field through the binding).
 """
 from __future__ import annotations
@@ -59,6 +60,21 @@ def main():
                          f"of the period, end {seg[-1]:.6f} K")
     with open(args.out + "_summary.txt", "w") as f:
         f.write("\n".join(lines) + "\n")
+    if tr.shape[0] and sim.batch > 1:
+        # parameter sweep: one row per batch member (the design-sweep table of configs[3])
+        cols = [np.arange(sim.batch), np.asarray(s["Q0"], dtype=np.float64)]
+        names = ["member", "Q0"]
+        if "heater_thickness_mm" in s:
+            cols.append(np.asarray(s["heater_thickness_mm"], dtype=np.float64))
+            names.append("heater_thickness_mm")
+        cols += [tr[:, :, 0].max(axis=0), tr[-1, :, 0]]
+        names += ["probe0_max_K", "probe0_end_K"]
+        np.savetxt(args.out + "_members.csv", np.c_[tuple(cols)], delimiter=",", fmt="%.9g", header=",".join(names))
+        k = int(np.argmax(cols[-2]))
+        lines.append(f"batch of {sim.batch}: probe 0 maximum over the run from {cols[-2].min():.6f} K to {cols[-2].max():.6f} K "
+                     f"(hottest member {k}: Q0 = {cols[1][k]:.4g})")
+        with open(args.out + "_summary.txt", "w") as f:
+            f.write("\n".join(lines) + "\n")
     if tr.shape[0]:
         idx = np.arange(0, tr.shape[0], max(1, args.every))
         np.savetxt(args.out + "_trace.csv", np.c_[idx, tr[idx, 0, :]], delimiter=",",
