@@ -215,8 +215,11 @@ const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, s
     if (getenv("HEAT_VARIANT")) return nullptr;
     if (const char *e = getenv("HEAT_KERNEL"))
         if (strcmp(e, "line") == 0 || strcmp(e, "tma") == 0) return nullptr;
-    // threads per CTA: 256 (two CTAs per SM) or 128 (four per SM); a line takes nr/8 threads
-    int NT = 256;
+    // threads per CTA: 256 (two CTAs per SM) or 128 (four per SM); a line takes nr/8 threads.
+    // Lines that fit 128 threads run best in CTAs of 128 (fewer independent lines share a barrier:
+    // 122 vs 104 GCUPS on configs[3], 133 vs 127 at nr = 1024); longer lines would need twice the
+    // cluster size (104 vs 123 GCUPS at nr = 2048) and stay at 256.
+    int NT = (d->nr <= 1024) ? 128 : 256;
     if (const char *e = getenv("HEAT_BAND_NT")) NT = (atoi(e) == 128) ? 128 : 256;
     if (d->nr != 512 && d->nr != 1024 && d->nr != 2048 && d->nr != 4096 && d->nr != 8192) return nullptr;
     const int G = std::min(d->nr / 8, NT), CL = d->nr / 8 / G;
