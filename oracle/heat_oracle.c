@@ -26,7 +26,11 @@
  *
  * Pins: tests/test_oracle_*.py (dense solve, discrete steady state, ln r, z-sine growth
  * factor, Bessel mode, lumped heating, energy identity, interface flux, schedule table,
- * tau-consistency with P:L278/L322).  Unpinned by the paper: reading G3 (face_mode), G9.
+ * tau-consistency with P:L278/L322) and, since round 2, tests/test_oracle_pins_r2.py: rows (13)
+ * re-assembled in NumPy (both face modes), the face_mode-1 rule on a hand-computed line and in
+ * the energy identity, probe records against the field of their step (bitwise).  Every function
+ * here has a pin.  What the PAPER cannot decide (both sides take the same reading): which of the
+ * two face rules G3 it means, and G9.
  */
 #include <math.h>
 #include <stdint.h>
