@@ -15,6 +15,7 @@
 #include "heat_line_kernel.cuh"
 #include "heat_tma_kernel.cuh"
 #include "heat_band_variants.h"
+#include "heat_wband_variants.h"
 
 using namespace heat;
 
@@ -267,12 +268,74 @@ const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, s
     return nullptr;
 }
 
+// The warp-autonomous band kernel (heat_wband_kernel.cuh) covers this descriptor iff a variant is
+// returned: what plan_band asks for, with 16-node chunks (at most one interface node per chunk).
+// Fills the chunk descriptors ([batch][nr/16]) when they are given.
+const WBandVariant *plan_wband(const heat_desc *d, std::vector<PLayer> *players, std::vector<uint32_t> *wdesc)
+{
+    if (getenv("HEAT_VARIANT")) return nullptr;
+    if (const char *e = getenv("HEAT_KERNEL"))
+        if (strcmp(e, "line") == 0 || strcmp(e, "tma") == 0 || strcmp(e, "band") == 0) return nullptr;
+    if (d->nr != 512 && d->nr != 1024 && d->nr != 2048 && d->nr != 4096 && d->nr != 8192) return nullptr;
+    if (d->face_mode != 0 || d->nz < 4) return nullptr;
+    const int nr = d->nr, N = nr - 1;
+    if (d->r[0] != 0.0) return nullptr;
+    const long double h = (long double)d->r[N] / (long double)N;
+    for (int i = 1; i <= N; ++i)
+        if (fabsl((long double)d->r[i] - h * i) > 1e-13L * (long double)d->r[N]) return nullptr;
+    int degk = 0;
+    std::vector<PLayer> pl((size_t)d->nlayers);
+    for (int m = 0; m < d->nlayers; ++m) {
+        int dk = 0;
+        if (!to_player(d->layers[m], &pl[(size_t)m], &dk)) return nullptr;
+        degk = std::max(degk, dk);
+    }
+    const int DEGK = degk <= 2 ? 2 : 4;
+    const int cpl = nr / 16;
+    std::vector<uint32_t> cd((size_t)d->batch * cpl, 0u);
+    for (int b = 0; b < d->batch; ++b) {
+        const uint8_t *seg = d->seg_layer + (size_t)b * (nr - 1);
+        for (int c = 0; c < cpl; ++c) {
+            const int i0 = 16 * c;
+            int ks = -1;
+            for (int k = 0; k < 16; ++k) {
+                const int i = i0 + k;
+                if (i >= 1 && i < N && seg[i - 1] != seg[i]) {
+                    if (ks >= 0) return nullptr; // two interface nodes in one chunk
+                    ks = k;
+                }
+            }
+            uint32_t A, B;
+            if (ks >= 0) { A = seg[i0 + ks - 1]; B = seg[i0 + ks]; }
+            else { A = B = seg[std::min(i0, N - 1)]; }
+            uint32_t w = A | (B << 8) | ((uint32_t)(ks + 1) << 16);
+            if (c == 0) w |= WD_FIRST;
+            if (c == cpl - 1) w |= WD_LAST;
+            cd[(size_t)b * cpl + c] = w;
+        }
+    }
+    const int WL = nr / 512;
+    int NW = 4;
+    if (const char *e = getenv("HEAT_WBAND_NW")) NW = atoi(e);
+    const WBandVariant *tab = DEGK == 2 ? k_wband_variants2 : k_wband_variants4;
+    const int ntab = DEGK == 2 ? k_nwband_variants2 : k_nwband_variants4;
+    const WBandVariant *found = nullptr;
+    for (int v = 0; v < ntab && !found; ++v)
+        if (tab[v].WL == WL && tab[v].NW == NW) found = &tab[v];
+    for (int v = 0; v < ntab && !found; ++v)
+        if (tab[v].WL == WL && tab[v].NW == 4) found = &tab[v];
+    if (!found) return nullptr;
+    if (players) *players = pl;
+    if (wdesc) *wdesc = cd;
+    return found;
+}
+
 constexpr int k_range_samples = 1025;
 
 // ---------------------------------------------------------------- workspace layout
 struct Layout {
     int nrp;
-    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, total;
+    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, off_wdesc, total;
 };
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -293,6 +356,7 @@ Layout make_layout(const heat_desc *d, const Variant *v, const TmaVariant *tv)
     L.off_cdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 16 + 1), 256);
     L.off_bdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 8 + 1), 256);
     L.off_players = o; o = align_up(o + sizeof(PLayer) * (size_t)HEAT_MAX_LAYERS, 256);
+    L.off_wdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 16 + 1), 256);
     L.total = o;
     return L;
 }
@@ -369,6 +433,9 @@ struct heat_ctx {
     const Variant *var;
     const TmaVariant *tvar; // non-NULL: heat_step launches the TMA kernel
     const BandVariant *bvar; // non-NULL: heat_step launches the band kernel
+    const WBandVariant *wvar; // non-NULL: heat_step launches the warp-autonomous band kernel (takes precedence)
+    WParams wp;
+    CUtensorMap wtm[2]; // [0] = field_a, [1] = field_b; box {16, 32}
     int pdl;                 // band kernel: launch with programmatic stream serialization
     CUtensorMap btm_ld[2], btm_st[2];
     BParams bp;
@@ -491,11 +558,13 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     for (int q = 0; q < c->nsub; ++q) c->amp_sub[(size_t)q] = 1.0 - std::exp(-(double)q / d->transient_k);
     std::vector<PLayer> players;
     std::vector<uint32_t> bdesc;
-    const BandVariant *bv = plan_band(d, &players, &bdesc);
-    c->var = v; c->tvar = tv; c->bvar = bv; c->lay = L; c->ws = (char *)workspace;
+    std::vector<uint32_t> wdesc;
+    const WBandVariant *wv = plan_wband(d, &players, &wdesc);
+    const BandVariant *bv = wv ? nullptr : plan_band(d, &players, &bdesc);
+    c->var = v; c->tvar = tv; c->bvar = bv; c->wvar = wv; c->lay = L; c->ws = (char *)workspace;
     // measured: 10.4 -> 8.7 us per step on 512 x 512, 36.9 -> 34.7 on 2048 x 2048; with clusters (nr >= 4096)
     // the piecemeal placement of the next step's clusters costs 11 %, so it stays off there
-    c->pdl = (bv && bv->CL == 1) ? 1 : 0;
+    c->pdl = ((bv && bv->CL == 1) || (wv && wv->CL == 1)) ? 1 : 0;
     if (const char *ep = getenv("HEAT_PDL")) c->pdl = atoi(ep) != 0;
     c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
@@ -633,6 +702,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     UP(L.off_cdesc, cdesc, uint32_t);
     if (bv) {
         UP(L.off_bdesc, bdesc, uint32_t);
+        UP(L.off_players, players, PLayer);
+    }
+    if (wv) {
+        UP(L.off_wdesc, wdesc, uint32_t);
         UP(L.off_players, players, PLayer);
     }
 #undef UP
@@ -816,6 +889,89 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         bp.rpl = nr / 16; bp.BL = best_BL; bp.bands_per_member = bpm; bp.total_bands = (int)bands;
     }
 
+    // ---- warp-autonomous band kernel: launch shape, band partition, tensor maps
+    if (wv) {
+        const size_t wsmem = wv->smem_fixed + sizeof(WLayer) * (size_t)d->nlayers;
+        const size_t wsmem_max = wv->smem_fixed + sizeof(WLayer) * (size_t)HEAT_MAX_LAYERS;
+        // the attribute belongs to the kernel function, not to this context: reserve the worst case
+        e = cudaFuncSetAttribute((const void *)wv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem_max);
+        if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", wv->name, wsmem_max, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        const int NT = 32 * wv->NW;
+        int max_clusters = 0;
+        {
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * (8 / wv->NW) * wv->CL), 1, 1);
+            cfg.blockDim = dim3((unsigned)NT, 1, 1);
+            cfg.dynamicSmemBytes = wsmem;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)wv->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            e = cudaOccupancyMaxActiveClusters(&max_clusters, (const void *)wv->fn, &cfg);
+            if (e != cudaSuccess || max_clusters < 1) { set_err(nullptr, "%s does not fit on the device (%s)", wv->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        }
+        if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / wv->CL);
+        // bands: every line group (LPB per CTA) walks BL consecutive lines of one batch member;
+        // choose the band count per member that minimises rounds * (BL + prologue)
+        const int LPB = wv->LPB, Lz = nz - 2;
+        const long long slots = (long long)max_clusters * LPB;
+        long long best_cost = -1;
+        int best_BL = Lz;
+        for (int nb = 1; nb <= Lz; ++nb) {
+            const int BL = (Lz + nb - 1) / nb;
+            const int bpm = (Lz + BL - 1) / BL;
+            const long long bands = (long long)d->batch * bpm;
+            const long long rounds = (bands + slots - 1) / slots;
+            const long long cost = rounds * (BL + 3);
+            if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_BL = BL; }
+        }
+        if (const char *eb = getenv("HEAT_BAND_LINES")) best_BL = std::max(1, std::min(Lz, atoi(eb)));
+        const int bpm = (Lz + best_BL - 1) / best_BL;
+        const long long bands = (long long)d->batch * bpm;
+        const long long nclusters = std::min<long long>((bands + LPB - 1) / LPB, max_clusters);
+        c->grid = (int)nclusters * wv->CL;
+        c->smem = wsmem;
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || !sym || qres != cudaDriverEntryPointSuccess) { set_err(nullptr, "cuTensorMapEncodeTiled is unavailable (%s)", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        encode_fn encode = (encode_fn)sym;
+        const cuuint64_t gdim[2] = {16, (cuuint64_t)cells / 16};
+        const cuuint64_t gstr[1] = {128};
+        const cuuint32_t estr[2] = {1, 1};
+        const cuuint32_t box[2] = {16, 32};
+        double *lev[2] = {c->cur, c->nxt};
+        for (int q = 0; q < 2; ++q) {
+            CUresult r1 = encode(&c->wtm[q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, lev[q], gdim, gstr, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r1 != CUDA_SUCCESS) { set_err(nullptr, "cuTensorMapEncodeTiled failed (%d)", (int)r1); return fail(HEAT_ECUDA); }
+        }
+        WParams &wp = c->wp;
+        memset(&wp, 0, sizeof wp);
+        wp.wdesc = (const uint32_t *)(c->ws + L.off_wdesc);
+        wp.players = (const PLayer *)(c->ws + L.off_players);
+        wp.ezm = (const double *)(c->ws + L.off_ezm);
+        wp.ezp = (const double *)(c->ws + L.off_ezp);
+        wp.Q0 = (const double *)(c->ws + L.off_q0);
+        wp.probes = (const ProbeSrc *)(c->ws + L.off_probes);
+        {
+            const long double h = ((long double)r[N] - (long double)r[0]) / (long double)N;
+            wp.g0 = (double)(1.0L / (h * h));
+        }
+        const bool din = d->r_in.kind == HEAT_BC_DIRICHLET, dout = d->r_out.kind == HEAT_BC_DIRICHLET;
+        wp.rin_om = din ? 1.0 : 0.0; wp.rin_be = din ? d->r_in.value : 0.0;
+        wp.rout_a = dout ? 0.0 : 1.0; wp.rout_w = dout ? 1.0 : 0.0; wp.rout_f = dout ? d->r_out.value : 0.0;
+        wp.nr = nr; wp.nz = nz; wp.batch = d->batch; wp.nlayers = d->nlayers; wp.nprobes = d->nprobes;
+        wp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
+        wp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
+        wp.rpl = nr / 16; wp.BL = best_BL; wp.bands_per_member = bpm; wp.total_bands = (int)bands;
+    }
+
     KParams &k = c->kp;
     memset(&k, 0, sizeof k);
     k.ga = (const double *)(c->ws + L.off_ga);
@@ -863,7 +1019,27 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
                 c->rec_dropped += 1;
             }
         }
-        if (c->bvar) {
+        if (c->wvar) {
+            const int q = (c->cur == c->field_a) ? 0 : 1;
+            WParams &wp = c->wp;
+            wp.tm_ld = c->wtm[q];
+            wp.tm_st = c->wtm[1 - q];
+            wp.Told = c->cur;
+            wp.inv_tau = k.inv_tau; wp.amp = k.amp; wp.probe_out = k.probe_out;
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)c->grid, 1, 1);
+            cfg.blockDim = dim3((unsigned)(32 * c->wvar->NW), 1, 1);
+            cfg.dynamicSmemBytes = c->smem;
+            cfg.stream = st;
+            cudaLaunchAttribute at[2];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)c->wvar->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            at[1].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = at; cfg.numAttrs = c->pdl ? 2 : 1;
+            CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->wvar->fn, wp));
+        } else if (c->bvar) {
             const int q = (c->cur == c->field_a) ? 0 : 1;
             BParams &bp = c->bp;
             bp.tm_ld = c->btm_ld[q];
@@ -956,7 +1132,7 @@ heat_status heat_probe(heat_ctx *c, double *dst_host, int64_t max, int64_t *n_wr
 
 int64_t heat_step_index(const heat_ctx *c) { return c ? c->step : -1; }
 int64_t heat_launch_count(const heat_ctx *c) { return c ? c->launches : -1; }
-const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->bvar ? c->bvar->name : c->tvar ? c->tvar->name : c->var->name) : ""; }
+const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->wvar ? c->wvar->name : c->bvar ? c->bvar->name : c->tvar ? c->tvar->name : c->var->name) : ""; }
 const char *heat_last_error(const heat_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
 void heat_destroy(heat_ctx *c) { delete c; }
 

@@ -249,9 +249,10 @@ def random_spec(seed, nr=13, nz=11, nlayers=3, batch=1, laws="mixed", source=Tru
 # ---------------------------------------------------------------- band-kernel edge cases
 
 def band_spec(seed, nr=512, nz=24, nlayers=4, batch=1, bcs=None, source=True, poly_laws=False,
-              nonuniform_z=True):
-    """Seeded problem on a uniform r grid starting at r = 0 (what the band kernel covers) with
-    interface nodes at every position of an 8-node chunk (first, last, middle), square-root,
+              nonuniform_z=True, chunk=8):
+    """Seeded problem on a uniform r grid starting at r = 0 (what the band kernels cover) with
+    interface nodes at every position of a thread's chunk of `chunk` nodes (first, last, middle;
+    8 nodes in the band kernel, 16 in the wband kernel), square-root,
     power and polynomial laws, random initial field, optional source and non-uniform z."""
     rng = np.random.Generator(np.random.PCG64(SEED + 1000 + int(seed)))
     R = 2e-3
@@ -272,9 +273,9 @@ def band_spec(seed, nr=512, nz=24, nlayers=4, batch=1, bcs=None, source=True, po
     segs = []
     for b in range(batch):
         # one interface per chosen chunk, at chunk positions 0, 7 and a random one
-        chunks = sorted(rng.choice(np.arange(1, nr // 8 - 1), size=nlayers - 1, replace=False).tolist())
-        pos = [0, 7] + [int(rng.integers(1, 7)) for _ in range(nlayers)]
-        nodes = [8 * c + pos[(q + b) % len(pos)] for q, c in enumerate(chunks)]
+        chunks = sorted(rng.choice(np.arange(1, nr // chunk - 1), size=nlayers - 1, replace=False).tolist())
+        pos = [0, chunk - 1] + [int(rng.integers(1, chunk - 1)) for _ in range(nlayers)]
+        nodes = [chunk * c + pos[(q + b) % len(pos)] for q, c in enumerate(chunks)]
         # adjacent chunks could give adjacent interface nodes (8c+7, 8c+8): move the second one
         for q in range(1, len(nodes)):
             if nodes[q] - nodes[q - 1] < 2:

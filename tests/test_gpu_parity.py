@@ -128,6 +128,7 @@ def test_band_kernel_edge_cases(bd, case, monkeypatch):
     z, random initial field, source with sub-steps, probes on boundary / interface / Dirichlet
     nodes, ragged band partition, clusters of 1, 2, 4 and 8 CTAs per line."""
     nr, nz, batch, poly, bcs, nt = case
+    monkeypatch.setenv("HEAT_KERNEL", "band")   # the third-generation kernel (wband takes precedence otherwise)
     monkeypatch.setenv("HEAT_BAND_NT", str(nt))
     s = I.band_spec(nr + nz, nr=nr, nz=nz, batch=batch, bcs=bcs, poly_laws=poly)
     s = with_dt(bd, s, 0.8)
@@ -144,11 +145,64 @@ def test_band_kernel_edge_cases(bd, case, monkeypatch):
     sim.close()
 
 
+WBAND_CASES = [
+    # nr, nz, batch, poly laws, bcs, HEAT_WBAND_NW
+    (512, 24, 3, False, None, 4),              # one warp per line, four lines per CTA
+    (512, 9, 5, True, BC_SETS[1], 4),          # 35 bands of 1..: ragged last round, Neumann z_lo
+    (1024, 21, 2, False, BC_SETS[2], 4),       # two warps per line, Dirichlet r boundaries
+    (2048, 19, 1, True, BC_SETS[3], 4),        # a CTA per line
+    (4096, 12, 1, False, None, 4),             # cluster of 2 CTAs per line
+    (8192, 7, 1, False, BC_SETS[1], 4),        # cluster of 4, Neumann z_lo
+    (8192, 6, 2, True, None, 2),               # cluster of 8 CTAs of 2 warps
+    (8192, 9, 1, False, BC_SETS[3], 8),        # cluster of 2 CTAs of 8 warps
+]
+
+
+@pytest.mark.parametrize("case", WBAND_CASES, ids=lambda c: f"nr{c[0]}-nz{c[1]}-b{c[2]}-{'poly' if c[3] else 'pow'}-nw{c[5]}")
+def test_wband_kernel_edge_cases(bd, case, monkeypatch):
+    """The warp-autonomous band kernel (the one bench.py times) on the band_spec problems:
+    interface nodes at the first / last / middle row of a thread's chunk, square root, power and
+    degree-4 polynomial laws side by side in one warp, every BC kind, non-uniform z, random
+    initial field, source with sub-steps, probes on boundary / interface / Dirichlet nodes,
+    ragged band partition, 1..16 warps per line in clusters of 1, 2, 4 and 8 CTAs."""
+    nr, nz, batch, poly, bcs, nw = case
+    monkeypatch.setenv("HEAT_WBAND_NW", str(nw))
+    s = I.band_spec(nr + nz, nr=nr, nz=nz, batch=batch, bcs=bcs, poly_laws=poly, chunk=16)
+    s = with_dt(bd, s, 0.8)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp" if nr * nz > 30000 else "double")
+    assert sim.kernel_name.startswith(f"wband<WL={nr // 512},NW={nw},"), sim.kernel_name
+    for n in (1, 6, 13):
+        sim.step(n)
+        orc.step(n)
+        compare(sim, orc)
+    pg, dropped = sim.probes()
+    po = orc.probes()
+    assert dropped == 0 and pg.shape == po.shape
+    assert np.max(np.abs(pg - po)) <= TOL
+    sim.close()
+
+
+def test_wband_kernel_band_length_does_not_change_the_result(bd, monkeypatch):
+    """The partition of the lines into bands is a scheduling choice: the field is bitwise the
+    same for bands of 1, 3 and all lines."""
+    s = with_dt(bd, I.band_spec(7, nr=1024, nz=20, batch=2, chunk=16), 0.8)
+    out = []
+    for bl in ("1", "3", "18"):
+        monkeypatch.setenv("HEAT_BAND_LINES", bl)
+        sim = bd.HeatSim(s)
+        assert sim.kernel_name.startswith("wband<"), sim.kernel_name
+        sim.step(9)
+        out.append(sim.fields())
+        sim.close()
+    assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
+
+
 def test_band_kernel_band_length_does_not_change_the_result(bd, monkeypatch):
     """The partition of the lines into bands is a scheduling choice: the field is bitwise the
     same for bands of 1, 3 and all lines."""
     s = with_dt(bd, I.band_spec(7, nr=512, nz=20, batch=2), 0.8)
     out = []
+    monkeypatch.setenv("HEAT_KERNEL", "band")
     for bl in ("1", "3", "18"):
         monkeypatch.setenv("HEAT_BAND_LINES", bl)
         sim = bd.HeatSim(s)
