@@ -24,7 +24,7 @@ HEAT_H = os.path.join(ROOT, "include", "heat.h")
 UNITS = {
     "heat_api.cu": _c("heat_api.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
                       "heat_band_params.cuh", "heat_band_variants.h", "heat_wband_params.cuh",
-                      "heat_wband_variants.h") + [HEAT_H],
+                      "heat_wband_variants.h", "heat_tband_variants.h") + [HEAT_H],
     "heat_band.cu": _c("heat_band.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
                        "heat_band_params.cuh", "heat_band_variants.h", "heat_band_kernel.cuh"),
     "heat_wband2.cu": _c("heat_wband2.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
@@ -33,6 +33,12 @@ UNITS = {
     "heat_wband4.cu": _c("heat_wband4.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
                          "heat_band_params.cuh", "heat_band_kernel.cuh", "heat_wband_params.cuh",
                          "heat_wband_variants.h", "heat_wband_kernel.cuh"),
+    "heat_tband2.cu": _c("heat_tband2.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                         "heat_band_params.cuh", "heat_band_kernel.cuh", "heat_wband_params.cuh",
+                         "heat_wband_kernel.cuh", "heat_tband_variants.h", "heat_tband_kernel.cuh"),
+    "heat_tband4.cu": _c("heat_tband4.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                         "heat_band_params.cuh", "heat_band_kernel.cuh", "heat_wband_params.cuh",
+                         "heat_wband_kernel.cuh", "heat_tband_variants.h", "heat_tband_kernel.cuh"),
 }
 SOURCES = _c(*UNITS)
 DEPS = sorted({d for deps in UNITS.values() for d in deps})

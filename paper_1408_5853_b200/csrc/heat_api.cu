@@ -16,6 +16,7 @@
 #include "heat_tma_kernel.cuh"
 #include "heat_band_variants.h"
 #include "heat_wband_variants.h"
+#include "heat_tband_variants.h"
 
 using namespace heat;
 
@@ -271,8 +272,10 @@ const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, s
 // The warp-autonomous band kernel (heat_wband_kernel.cuh) covers this descriptor iff a variant is
 // returned: what plan_band asks for, with 16-node chunks (at most one interface node per chunk).
 // Fills the chunk descriptors ([batch][nr/16]) when they are given.
-const WBandVariant *plan_wband(const heat_desc *d, std::vector<PLayer> *players, std::vector<uint32_t> *wdesc)
+const WBandVariant *plan_wband(const heat_desc *d, std::vector<PLayer> *players, std::vector<uint32_t> *wdesc,
+                               const TBandVariant **tband)
 {
+    if (tband) *tband = nullptr;
     if (getenv("HEAT_VARIANT")) return nullptr;
     if (const char *e = getenv("HEAT_KERNEL"))
         if (strcmp(e, "line") == 0 || strcmp(e, "tma") == 0 || strcmp(e, "band") == 0) return nullptr;
@@ -325,6 +328,19 @@ const WBandVariant *plan_wband(const heat_desc *d, std::vector<PLayer> *players,
     for (int v = 0; v < ntab && !found; ++v)
         if (tab[v].WL == WL && tab[v].NW == 4) found = &tab[v];
     if (!found) return nullptr;
+    // the tensor-memory version of the same kernel (16 warps per SM) unless HEAT_KERNEL=wband asks for
+    // the register version
+    const char *ek = getenv("HEAT_KERNEL");
+    if (tband && !(ek && strcmp(ek, "wband") == 0)) {
+        int TNW = 4;
+        if (const char *e = getenv("HEAT_TBAND_NW")) TNW = atoi(e);
+        const TBandVariant *ttab = DEGK == 2 ? k_tband_variants2 : k_tband_variants4;
+        const int nttab = DEGK == 2 ? k_ntband_variants2 : k_ntband_variants4;
+        for (int v = 0; v < nttab && !*tband; ++v)
+            if (ttab[v].WL == WL && ttab[v].NW == TNW) *tband = &ttab[v];
+        for (int v = 0; v < nttab && !*tband; ++v)
+            if (ttab[v].WL == WL && ttab[v].NW == 4) *tband = &ttab[v];
+    }
     if (players) *players = pl;
     if (wdesc) *wdesc = cd;
     return found;
@@ -434,6 +450,7 @@ struct heat_ctx {
     const TmaVariant *tvar; // non-NULL: heat_step launches the TMA kernel
     const BandVariant *bvar; // non-NULL: heat_step launches the band kernel
     const WBandVariant *wvar; // non-NULL: heat_step launches the warp-autonomous band kernel (takes precedence)
+    const TBandVariant *tbvar; // non-NULL: ... its tensor-memory version (takes precedence over wvar)
     WParams wp;
     CUtensorMap wtm[2]; // [0] = field_a, [1] = field_b; box {16, 32}
     int pdl;                 // band kernel: launch with programmatic stream serialization
@@ -559,12 +576,13 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     std::vector<PLayer> players;
     std::vector<uint32_t> bdesc;
     std::vector<uint32_t> wdesc;
-    const WBandVariant *wv = plan_wband(d, &players, &wdesc);
+    const TBandVariant *tbv = nullptr;
+    const WBandVariant *wv = plan_wband(d, &players, &wdesc, &tbv);
     const BandVariant *bv = wv ? nullptr : plan_band(d, &players, &bdesc);
-    c->var = v; c->tvar = tv; c->bvar = bv; c->wvar = wv; c->lay = L; c->ws = (char *)workspace;
+    c->var = v; c->tvar = tv; c->bvar = bv; c->wvar = wv; c->tbvar = tbv; c->lay = L; c->ws = (char *)workspace;
     // measured: 10.4 -> 8.7 us per step on 512 x 512, 36.9 -> 34.7 on 2048 x 2048; with clusters (nr >= 4096)
     // the piecemeal placement of the next step's clusters costs 11 %, so it stays off there
-    c->pdl = ((bv && bv->CL == 1) || (wv && wv->CL == 1)) ? 1 : 0;
+    c->pdl = ((bv && bv->CL == 1) || (wv && !tbv && wv->CL == 1)) ? 1 : 0;
     if (const char *ep = getenv("HEAT_PDL")) c->pdl = atoi(ep) != 0;
     c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
@@ -891,30 +909,42 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
 
     // ---- warp-autonomous band kernel: launch shape, band partition, tensor maps
     if (wv) {
-        const size_t wsmem = wv->smem_fixed + sizeof(WLayer) * (size_t)d->nlayers;
-        const size_t wsmem_max = wv->smem_fixed + sizeof(WLayer) * (size_t)HEAT_MAX_LAYERS;
+        // the register version (wband) and the tensor-memory version (tband) share parameters and band
+        // partition; they differ in warps per SM (8 / 16) and shared memory
+        const void *wfn = tbv ? (const void *)tbv->fn : (const void *)wv->fn;
+        const char *wname = tbv ? tbv->name : wv->name;
+        const size_t wfixed = tbv ? tbv->smem_fixed : wv->smem_fixed;
+        const int wNW = tbv ? tbv->NW : wv->NW, wCL = tbv ? tbv->CL : wv->CL, wLPB = tbv ? tbv->LPB : wv->LPB;
+        const int warps_per_sm = tbv ? 16 : 8;
+        const size_t wsmem = wfixed + sizeof(WLayer) * (size_t)d->nlayers;
+        const size_t wsmem_max = wfixed + sizeof(WLayer) * (size_t)HEAT_MAX_LAYERS;
         // the attribute belongs to the kernel function, not to this context: reserve the worst case
-        e = cudaFuncSetAttribute((const void *)wv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem_max);
-        if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", wv->name, wsmem_max, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
-        const int NT = 32 * wv->NW;
+        e = cudaFuncSetAttribute(wfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsmem_max);
+        if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", wname, wsmem_max, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+        const int NT = 32 * wNW;
         int max_clusters = 0;
         {
             cudaLaunchConfig_t cfg;
             memset(&cfg, 0, sizeof cfg);
-            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * (8 / wv->NW) * wv->CL), 1, 1);
+            cfg.gridDim = dim3((unsigned)(prop.multiProcessorCount * (warps_per_sm / wNW) * wCL), 1, 1);
             cfg.blockDim = dim3((unsigned)NT, 1, 1);
             cfg.dynamicSmemBytes = wsmem;
             cudaLaunchAttribute at[1];
             at[0].id = cudaLaunchAttributeClusterDimension;
-            at[0].val.clusterDim.x = (unsigned)wv->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            at[0].val.clusterDim.x = (unsigned)wCL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
             cfg.attrs = at; cfg.numAttrs = 1;
-            e = cudaOccupancyMaxActiveClusters(&max_clusters, (const void *)wv->fn, &cfg);
-            if (e != cudaSuccess || max_clusters < 1) { set_err(nullptr, "%s does not fit on the device (%s)", wv->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+            e = cudaOccupancyMaxActiveClusters(&max_clusters, wfn, &cfg);
+            if (e != cudaSuccess || max_clusters < 1) { set_err(nullptr, "%s does not fit on the device (%s)", wname, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
         }
-        if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / wv->CL);
+        // tensor memory: the CTAs of an SM share 512 columns, 128 per four warps, so exactly 16 / NW CTAs
+        // fit.  (The occupancy query reports a single CTA per SM for a kernel that executes
+        // tcgen05.alloc although 16 / NW are resident; registers (128) and shared memory (<= 52 KB per
+        // four warps) allow them, see the static_asserts in heat_tband_kernel.cuh.)
+        if (tbv) max_clusters = prop.multiProcessorCount * (warps_per_sm / wNW) / wCL;
+        if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / wCL);
         // bands: every line group (LPB per CTA) walks BL consecutive lines of one batch member;
         // choose the band count per member that minimises rounds * (BL + prologue)
-        const int LPB = wv->LPB, Lz = nz - 2;
+        const int LPB = wLPB, Lz = nz - 2;
         const long long slots = (long long)max_clusters * LPB;
         long long best_cost = -1;
         int best_BL = Lz;
@@ -930,7 +960,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         const int bpm = (Lz + best_BL - 1) / best_BL;
         const long long bands = (long long)d->batch * bpm;
         const long long nclusters = std::min<long long>((bands + LPB - 1) / LPB, max_clusters);
-        c->grid = (int)nclusters * wv->CL;
+        c->grid = (int)nclusters * wCL;
         c->smem = wsmem;
         typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                       const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -1029,16 +1059,18 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
             cudaLaunchConfig_t cfg;
             memset(&cfg, 0, sizeof cfg);
             cfg.gridDim = dim3((unsigned)c->grid, 1, 1);
-            cfg.blockDim = dim3((unsigned)(32 * c->wvar->NW), 1, 1);
+            const int lNW = c->tbvar ? c->tbvar->NW : c->wvar->NW, lCL = c->tbvar ? c->tbvar->CL : c->wvar->CL;
+            cfg.blockDim = dim3((unsigned)(32 * lNW), 1, 1);
             cfg.dynamicSmemBytes = c->smem;
             cfg.stream = st;
             cudaLaunchAttribute at[2];
             at[0].id = cudaLaunchAttributeClusterDimension;
-            at[0].val.clusterDim.x = (unsigned)c->wvar->CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            at[0].val.clusterDim.x = (unsigned)lCL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
             at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
             at[1].val.programmaticStreamSerializationAllowed = 1;
             cfg.attrs = at; cfg.numAttrs = c->pdl ? 2 : 1;
-            CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->wvar->fn, wp));
+            if (c->tbvar) CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->tbvar->fn, wp));
+            else CUDA_TRY(&c->err, cudaLaunchKernelEx(&cfg, c->wvar->fn, wp));
         } else if (c->bvar) {
             const int q = (c->cur == c->field_a) ? 0 : 1;
             BParams &bp = c->bp;
@@ -1132,7 +1164,7 @@ heat_status heat_probe(heat_ctx *c, double *dst_host, int64_t max, int64_t *n_wr
 
 int64_t heat_step_index(const heat_ctx *c) { return c ? c->step : -1; }
 int64_t heat_launch_count(const heat_ctx *c) { return c ? c->launches : -1; }
-const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->wvar ? c->wvar->name : c->bvar ? c->bvar->name : c->tvar ? c->tvar->name : c->var->name) : ""; }
+const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->tbvar ? c->tbvar->name : c->wvar ? c->wvar->name : c->bvar ? c->bvar->name : c->tvar ? c->tvar->name : c->var->name) : ""; }
 const char *heat_last_error(const heat_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
 void heat_destroy(heat_ctx *c) { delete c; }
 

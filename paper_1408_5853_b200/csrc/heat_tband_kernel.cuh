@@ -1,0 +1,578 @@
+// heat_tband_kernel.cuh -- fifth-generation fused time-step kernel for sm_100a: the warp-autonomous
+// band kernel (heat_wband_kernel.cuh) with the sweep coefficients parked in TENSOR MEMORY.
+//
+// Why: heat_wband_kernel is purely latency-bound -- its throughput on 8192 x 8192 is proportional
+// to the warps per SM (4 warps: 60, 6: 88, 8: 113 GCUPS, profiles/r02_wband_scaling.md) -- and the
+// 96 registers that hold (alpha, beta, gamma) of a thread's 16 rows between the forward sweep (12)
+// and the back substitution (14) cap it at 8 warps per SM.  Blackwell's tensor memory gives every
+// thread of a warp a private 512-byte strip (its lane x 128 columns of 32 bits): exactly 16 rows x
+// (alpha, beta, gamma, face flux).  With those parked there (tcgen05.st during the sweep,
+// tcgen05.ld during the back substitution) the kernel needs <= 128 registers and three 4 KB line
+// slots per warp, so 16 warps = 8192 nodes x 16 B of state are in flight per SM: a whole line of
+// the large grid, in four independent CTAs whose waits overlap.
+// Everything else (one branch-free row loop, per-warp TMA pipelines, separator exchange by
+// st.async + mbarrier) is as in heat_wband_kernel.cuh; same coverage, same arithmetic.
+// "P:Lnnn" cites a line of the paper text; readings G1..G22 are listed in DESIGN.md.
+#pragma once
+#include <cuda.h>
+
+#include "heat_wband_kernel.cuh"
+
+namespace heat {
+
+// WL = warps per line (nr = 512 WL), NW = warps per CTA (4, 8 or 16: every lane quarter of the
+// tensor memory is used).  16 / NW CTAs per SM.
+template <int WL, int NW>
+struct TBandCfg {
+    static constexpr int M = 16;
+    static constexpr int NT = 32 * NW;
+    static constexpr int CL = (WL > NW) ? WL / NW : 1;
+    static constexpr int LPB = (WL < NW) ? NW / WL : 1;
+    static constexpr int WPL = (WL < NW) ? WL : NW;
+    static constexpr int NS = 3;                      // ring of staged line parts per warp: j, j+1, j+2
+    static constexpr int SLOT = 4096;                 // 32 threads x 16 doubles
+    static constexpr int PUB = 12;
+    static constexpr int TCOLS = 128 * (NW / 4);      // tensor-memory columns of the CTA
+    static constexpr int WARP_BYTES = NS * SLOT;
+    static constexpr int OFF_HALO = NW * WARP_BYTES;                  // [NW][NS][4 doubles]
+    static constexpr int OFF_PUB = OFF_HALO + NW * NS * 32;           // [2][LPB][WL][PUB]
+    static constexpr int OFF_FBAR = OFF_PUB + 2 * LPB * WL * PUB * 8; // [NW][NS] load barriers
+    static constexpr int OFF_XBAR = OFF_FBAR + NW * NS * 8;           // [LPB][2] exchange barriers
+    static constexpr int OFF_TMEM = OFF_XBAR + LPB * 2 * 8;           // tensor-memory base address
+    static constexpr int OFF_LAY = OFF_TMEM + 16;
+    static constexpr size_t smem_bytes(int nlayers) { return 1024 + (size_t)OFF_LAY + sizeof(WLayer) * (size_t)nlayers; }
+};
+
+// ---------------------------------------------------------------- tensor memory as a register file
+// A warp addresses its own lane quarter; lane i of the warp owns tensor-memory lane (quarter*32 + i),
+// `x8` moves eight consecutive 32-bit columns = four doubles per thread.
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, double a, double b, double c, double d)
+{
+    asm volatile("{\n\t.reg .b32 r<8>;\n\t"
+                 "mov.b64 {r0, r1}, %1;\n\tmov.b64 {r2, r3}, %2;\n\tmov.b64 {r4, r5}, %3;\n\tmov.b64 {r6, r7}, %4;\n\t"
+                 "tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {r0, r1, r2, r3, r4, r5, r6, r7};\n\t}"
+                 ::"r"(taddr), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+struct TRaw8 {
+    uint32_t r[8];
+};
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, TRaw8 &v)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v.r[0]), "=r"(v.r[1]), "=r"(v.r[2]), "=r"(v.r[3]), "=r"(v.r[4]), "=r"(v.r[5]), "=r"(v.r[6]), "=r"(v.r[7])
+                 : "r"(taddr) : "memory");
+}
+// the loaded registers are valid only after the wait: they pass through it as operands so that no
+// use can be scheduled ahead of it
+__device__ __forceinline__ void tmem_wait_ld(TRaw8 &v)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(v.r[0]), "+r"(v.r[1]), "+r"(v.r[2]), "+r"(v.r[3]), "+r"(v.r[4]), "+r"(v.r[5]), "+r"(v.r[6]), "+r"(v.r[7])
+                 :: "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld3(TRaw8 &a, TRaw8 &b, TRaw8 &c)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(a.r[0]), "+r"(a.r[1]), "+r"(a.r[2]), "+r"(a.r[3]), "+r"(a.r[4]), "+r"(a.r[5]), "+r"(a.r[6]), "+r"(a.r[7]),
+                   "+r"(b.r[0]), "+r"(b.r[1]), "+r"(b.r[2]), "+r"(b.r[3]), "+r"(b.r[4]), "+r"(b.r[5]), "+r"(b.r[6]), "+r"(b.r[7]),
+                   "+r"(c.r[0]), "+r"(c.r[1]), "+r"(c.r[2]), "+r"(c.r[3]), "+r"(c.r[4]), "+r"(c.r[5]), "+r"(c.r[6]), "+r"(c.r[7])
+                 :: "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ double traw(const TRaw8 &v, int n) { return __hiloint2double((int)v.r[2 * n + 1], (int)v.r[2 * n]); }
+
+// columns of a thread's strip: rows in groups of four, group g: 24 columns of (alpha, beta, gamma) x 4
+// at 24 g, the four face fluxes at 96 + 8 g
+__device__ __forceinline__ constexpr uint32_t tcol_coef(int g, int part) { return (uint32_t)(24 * g + 8 * part); }
+__device__ __forceinline__ constexpr uint32_t tcol_flux(int g) { return (uint32_t)(96 + 8 * g); }
+
+struct TSweepArgs {
+    uint32_t sc, su;         // shared addresses: line j, line j+1
+    uint32_t tm;             // tensor-memory address of the warp's strip (column 0)
+    uint32_t rowo, sw;       // byte offset of the thread's tensor row in a slot, its swizzle phase
+    uint32_t layA, layB;     // shared addresses of the WLayer before / from the interface row on
+    double hl, hr;           // r neighbours of the chunk at line j
+    double fi0, g0, ezp, ezm;
+    double gl0;              // geometric factor of the face i0 - 1/2 (0 in the chunk that starts with a Neumann r_in row)
+    double fie15;            // capacity / rhs factor of row 15 (0 in the chunk that ends with a Neumann r_out row)
+    double qsA, qsB;         // source term X (2)-(4),(22) of the two layers
+    int ks;                  // interface row (18) of this chunk, < 0: none
+    bool sqA, sqB;
+    bool din, dout;          // the chunk starts / ends with a Dirichlet r-boundary row
+    bool nin, last;          // the chunk starts with the Neumann r_in row / ends with the r_out row
+    double rin_be, rout_f;
+};
+
+// what the reduced system needs from a thread's sweep
+struct TSweepOut {
+    double P, Q, S;          // x_first = P x_last + Q + S u
+    double al, be, gm;       // last row: x_last = al x_next + be + gm u
+};
+
+// law coefficients of one row, read from the shared table (layer A before the interface row, layer B
+// from it on: the face i* + 1/2 belongs to layer B, G14).  All lanes but the one that holds an
+// interface node read the same address, so these are broadcast loads; fetching them per row keeps
+// them out of the long-lived registers and needs no branch.
+template <int DEGK>
+struct TRowCoef {
+    double K[DEGK + 1];
+    double Ct[4];
+};
+template <int DEGK>
+__device__ __forceinline__ TRowCoef<DEGK> trow_coef(uint32_t a)
+{
+    TRowCoef<DEGK> c;
+    const double2 k01 = lds128(a);
+    c.K[0] = k01.x; c.K[1] = k01.y;
+    if (DEGK == 2) {
+        c.K[2] = lds64(a + 16);
+    } else {
+        const double2 k23 = lds128(a + 16);
+        c.K[2] = k23.x; c.K[3] = k23.y;
+        c.K[DEGK] = lds64(a + 32);
+    }
+    const double2 c01 = lds128(a + 48), c23 = lds128(a + 64);
+    c.Ct[0] = c01.x; c.Ct[1] = c01.y; c.Ct[2] = c23.x; c.Ct[3] = c23.y;
+    return c;
+}
+
+// Level 1 for one thread: rows (13) P:L140-145 assembled and pushed through the sweep (12)
+// P:L133-136, sixteen rows in four groups of four; (alpha, beta, gamma) and the new face fluxes of a
+// group go to tensor memory, the prefix products for the reduced row are carried along.  Special
+// rows as in wsweep16 (heat_wband_kernel.cuh): no branch inside the row loop.
+template <int DEGK, bool SQ>
+__device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, const uint32_t (&co)[8])
+{
+    SweepState st;
+    st.om = 1.0; st.be = 0.0; st.gm = 1.0;
+    TSweepOut o;
+    o.P = 1.0; o.Q = 0.0; o.S = 0.0;
+    // interface node: lam*_A, lam*_B at T_{i*,j} of the old level
+    double lamA_if = 0.0, lamB_if = 0.0;
+    if (A.ks >= 0) {
+        const double Tk = lds64(A.sc + A.rowo + ((((uint32_t)A.ks >> 1) ^ A.sw) << 4) + (((uint32_t)A.ks & 1u) << 3));
+        const TRowCoef<DEGK> ca = trow_coef<DEGK>(A.layA), cb = trow_coef<DEGK>(A.layB);
+        lamA_if = wlam<DEGK, true>(ca.K, A.sqA, Tk + Tk);
+        lamB_if = wlam<DEGK, true>(cb.K, A.sqB, Tk + Tk);
+    }
+    const uint32_t ksw = (A.ks >= 0) ? (uint32_t)A.ks : 99u;
+    TRaw8 fraw;
+    tmem_ld8(A.tm + tcol_flux(0), fraw);
+    double2 tl = lds128(A.sc + co[0]);
+    {
+        const TRowCoef<DEGK> c0 = trow_coef<DEGK>(A.layA);
+        st.cfL = wlam<DEGK, SQ>(c0.K, A.sqA, A.hl + tl.x) * A.gl0; // face i0 - 1/2
+    }
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+        tmem_wait_ld(fraw);
+        double fD[4];
+#pragma unroll
+        for (int n = 0; n < 4; ++n) fD[n] = traw(fraw, n);
+        if (g < 3) tmem_ld8(A.tm + tcol_flux(g < 3 ? g + 1 : 3), fraw);
+        double cf[12], fu[4];
+        double2 tn, tu;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int k = 4 * g + r, qq = k >> 1, e = k & 1;
+            double T, Tr, Tu;
+            if (e == 0) { // tl holds (T_k, T_{k+1})
+                tu = lds128(A.su + co[qq]);
+                T = tl.x; Tr = tl.y; Tu = tu.x;
+            } else {
+                if (qq < 7) tn = lds128(A.sc + co[qq < 7 ? qq + 1 : 7]);
+                else tn = make_double2(A.hr, A.hr);
+                T = tl.y; Tr = tn.x; Tu = tu.y;
+            }
+            const bool isB = ((uint32_t)k >= ksw);
+            const bool isif = ((uint32_t)k == ksw);
+            const TRowCoef<DEGK> c = trow_coef<DEGK>(isB ? A.layB : A.layA);
+            const double qs = isB ? A.qsB : A.qsA;
+            const bool sq = isB ? A.sqB : A.sqA;
+            const double fi = A.fi0 + (double)k;
+            double fie = (k == 15) ? A.fie15 : fi;
+            fie = isif ? 0.0 : fie;
+            double cfR, w, f;
+            wrow2<DEGK, SQ>(c.K, c.Ct, qs, sq, T, Tr, Tu, fD[r], fi, fie, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
+            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
+            double cfL_use = isif ? lamA_if : st.cfL;
+            double cfR_use = isif ? lamB_if : cfR;
+            if (k == 15) { // r_out row (15),(17): x_N = x_{N-1} (fie15 = 0, no right face) or x_N = value
+                cfR_use = A.last ? 0.0 : cfR_use;
+                cfL_use = A.dout ? 0.0 : cfL_use;
+                w = A.dout ? 1.0 : w;
+                f = A.dout ? A.rout_f : f;
+            }
+            st.cfL = cfL_use;
+            double alk;
+            sweep_row(st, cfR_use, w, f, alk);
+            st.cfL = cfR; // face i + 1/2 as the next regular row sees it
+            if (k == 0) { // r_in row (15),(16): alpha_0 = 1 exactly (T^_0 = T^_1 bitwise); Dirichlet: x_0 = value
+                alk = A.nin ? 1.0 : alk;
+                alk = A.din ? 0.0 : alk;
+                st.om = A.din ? 1.0 : st.om;
+                st.be = A.din ? A.rin_be : st.be;
+                st.gm = A.din ? 0.0 : st.gm;
+            }
+            cf[3 * r] = alk; cf[3 * r + 1] = st.be; cf[3 * r + 2] = st.gm;
+            if (k < 15) { // x_0 = P x_{k+1} + Q + S u
+                o.Q = fma(o.P, st.be, o.Q);
+                o.S = fma(o.P, st.gm, o.S);
+                o.P = o.P * alk;
+            }
+            if (e == 1) tl = tn;
+        }
+        tmem_st4(A.tm + tcol_coef(g, 0), cf[0], cf[1], cf[2], cf[3]);
+        tmem_st4(A.tm + tcol_coef(g, 1), cf[4], cf[5], cf[6], cf[7]);
+        tmem_st4(A.tm + tcol_coef(g, 2), cf[8], cf[9], cf[10], cf[11]);
+        tmem_st4(A.tm + tcol_flux(g), fu[0], fu[1], fu[2], fu[3]);
+        if (g == 3) { o.al = cf[9]; o.be = cf[10]; o.gm = cf[11]; }
+    }
+    return o;
+}
+
+template <int WL, int NW, int DEGK>
+__global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __grid_constant__ WParams p)
+{
+    using Cfg = TBandCfg<WL, NW>;
+    constexpr int CL = Cfg::CL, LPB = Cfg::LPB, WPL = Cfg::WPL, NS = Cfg::NS, SLOT = Cfg::SLOT;
+    constexpr uint32_t FULL = 0xffffffffu;
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char *gbase = smem_raw + (sbase - smem_u32(smem_raw));
+    WLayer *lay = reinterpret_cast<WLayer *>(gbase + Cfg::OFF_LAY);
+    volatile uint32_t *tmem_slot = reinterpret_cast<volatile uint32_t *>(gbase + Cfg::OFF_TMEM);
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int warp = __shfl_sync(FULL, tid >> 5, 0); // provably warp-uniform: TMA operands stay in uniform registers
+    const int grp = warp / WPL; // line (band) within the CTA
+    const int wl = warp % WPL;  // warp within the CTA's part of the line
+    const int cluster_id = blockIdx.x / CL, nclusters = gridDim.x / CL;
+    // rank of this CTA within the line: the hardware rank, rotated by CL/2 in odd clusters so that
+    // the CTAs sharing an SM do not hold the same (possibly most expensive) part of the radius
+    const int crank = (CL > 1) ? (int)((cluster_ctarank() + (uint32_t)((cluster_id & 1) ? CL / 2 : 0)) % (uint32_t)CL) : 0;
+    const int wig = crank * WPL + wl; // warp within the line = separator index
+    const int t = wig * 32 + lane;    // thread within the line = tensor row within the line
+    const int i0 = t * 16;
+    const uint32_t wbase = sbase + (uint32_t)warp * (uint32_t)Cfg::WARP_BYTES;
+    const uint32_t halo_a = sbase + Cfg::OFF_HALO + (uint32_t)(warp * NS) * 32u;
+    const uint32_t fbar_a = sbase + Cfg::OFF_FBAR + (uint32_t)(warp * NS) * 8u;
+    const uint32_t xbar_a = sbase + Cfg::OFF_XBAR + (uint32_t)grp * 16u;
+    const uint32_t pub_a = sbase + Cfg::OFF_PUB;
+    // byte offsets of the thread's eight 16-byte chunks inside a SWIZZLE_128B slot, and of its two
+    // r neighbours (last node of the row above, first node of the row below)
+    uint32_t co[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) co[q] = (uint32_t)lane * 128u + (uint32_t)((q ^ (lane & 7)) << 4);
+    const uint32_t hlo = (uint32_t)(lane - 1) * 128u + (uint32_t)((7 ^ ((lane - 1) & 7)) << 4) + 8u;
+    const uint32_t hro = (uint32_t)(lane + 1) * 128u + (uint32_t)(((lane + 1) & 7) << 4);
+    const bool has_l = (wig > 0), has_r = (wig < WL - 1); // the warp has a left / right neighbour warp
+
+    // ---- law table scaled for this launch, barriers, tensor memory
+    if (tid < p.nlayers) {
+        const PLayer &P = p.players[tid];
+        WLayer W;
+#pragma unroll
+        for (int n = 0; n < 5; ++n) W.K[n] = P.K[n];
+        W.K[5] = 0.0;
+#pragma unroll
+        for (int n = 0; n < 4; ++n) W.Ct[n] = P.C[n] * p.inv_tau;
+        W.qsrc = P.heater ? p.amp * P.src : 0.0;
+        W.sq = P.sqrtk;
+        W.pad_ = 0;
+        lay[tid] = W;
+    }
+    if (tid == 0) {
+#pragma unroll 1
+        for (int s = 0; s < NW * NS; ++s) mbar_init(sbase + Cfg::OFF_FBAR + 8u * s, 1);
+#pragma unroll 1
+        for (int s = 0; s < LPB * 2; ++s) mbar_init(sbase + Cfg::OFF_XBAR + 8u * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     ::"r"(sbase + (uint32_t)Cfg::OFF_TMEM), "n"(Cfg::TCOLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_base = *tmem_slot;
+    // the warp's strip: lane quarter warp % 4, 128 columns per group of four warps
+    const uint32_t tm = tmem_base + ((uint32_t)(warp & 3) << 21) + (uint32_t)(warp >> 2) * 128u;
+    if (CL > 1) { cluster_arrive(); cluster_wait(); }
+    // programmatic dependent launch: the set-up above overlaps the tail of the previous step
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+    const int nz = p.nz, rpl = p.rpl, BL = p.BL, bpm = p.bands_per_member;
+    const double g0 = p.g0;
+    double fi0 = (double)i0;
+    uint32_t qbase = 0;  // load sequence number of line offset -1 of this band
+    uint32_t lcount = 0; // lines done (phase of the exchange barriers)
+
+    for (int round = 0;; ++round) {
+        const int band = (round * nclusters + cluster_id) * LPB + grp;
+        if (band >= p.total_bands) break; // uniform over the warps of a line
+        const int b = band / bpm;
+        const int j0 = 1 + (band - b * bpm) * BL;
+        const int j1 = min(j0 + BL, nz - 1);
+        const int nl = j1 - j0;
+        const int row0 = (b * nz + j0 - 1) * rpl + wig * 32; // tensor row of this warp's part of line j0 - 1
+
+        // load sequence s (line j0 - 1 + s) -> slot s % NS; lane 0 issues every TMA operation of the warp
+        auto issue_load = [&](uint32_t s) {
+            const uint32_t q = qbase + s, sl = q % (uint32_t)NS;
+            const uint32_t bar = fbar_a + 8u * sl;
+            const int R = row0 + (int)s * rpl;
+            mbar_expect_tx(bar, (uint32_t)SLOT + (has_l ? 16u : 0u) + (has_r ? 16u : 0u));
+            tma_load_2d(wbase + sl * (uint32_t)SLOT, &p.tm_ld, 0, R, bar);
+            const double *g = p.Told + (size_t)R * 16;
+            if (has_l) bulk_load_16(halo_a + sl * 32u, g - 2, bar);
+            if (has_r) bulk_load_16(halo_a + sl * 32u + 16u, g + 512, bar);
+        };
+        auto wait_seq = [&](uint32_t s) {
+            const uint32_t q = qbase + s;
+            while (!mbar_try_wait(fbar_a + 8u * (q % (uint32_t)NS), (q / (uint32_t)NS) & 1u)) {}
+        };
+
+        // ---- per-thread constants of this band
+        const uint32_t cd = __ldg(p.wdesc + (size_t)b * rpl + t);
+        const int la = (int)(cd & 0xffu), lb = (int)((cd >> 8) & 0xffu);
+        const int ks = (int)((cd >> 16) & 0x1fu) - 1;
+        const bool first = (cd & WD_FIRST) != 0, last = (cd & WD_LAST) != 0;
+        const double q0b = __ldg(p.Q0 + b); // X = Q0 nu(t_k) p^2(t_k) s, (2)-(4),(22)
+        const bool rin_neu = (p.rin_om == 0.0), rout_neu = (p.rout_w == 0.0);
+        TSweepArgs A;
+        A.tm = tm; A.rowo = (uint32_t)lane * 128u; A.sw = (uint32_t)lane & 7u;
+        A.layA = smem_u32(&lay[la]); A.layB = smem_u32(&lay[lb]);
+        A.g0 = g0;
+        A.gl0 = (first && rin_neu) ? 0.0 : fma(g0, (double)i0, -0.5 * g0);
+        A.fie15 = (last && rout_neu) ? 0.0 : (double)(i0 + 15);
+        A.qsA = lay[la].qsrc * q0b; A.qsB = lay[lb].qsrc * q0b;
+        A.sqA = (lay[la].sq != 0); A.sqB = (lay[lb].sq != 0);
+        A.ks = ks; A.din = first && !rin_neu; A.dout = last && !rout_neu; A.nin = first && rin_neu; A.last = last;
+        A.rin_be = p.rin_be; A.rout_f = p.rout_f;
+        const bool anysq = __any_sync(FULL, A.sqA || (ks >= 0 && A.sqB));
+
+        if (lane == 0) {
+            const uint32_t npre = (uint32_t)min(NS, nl + 2);
+            for (uint32_t s = 0; s < npre; ++s) issue_load(s);
+        }
+        wait_seq(0);
+        wait_seq(1);
+
+        // ---- prologue: the flux through the faces between lines j0 - 1 and j0, into tensor memory
+        {
+            const uint32_t sd = wbase + ((qbase + 0u) % (uint32_t)NS) * (uint32_t)SLOT;
+            const uint32_t s1 = wbase + ((qbase + 1u) % (uint32_t)NS) * (uint32_t)SLOT;
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                double fl[4];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int q = 2 * g + h;
+                    const double2 td = lds128(sd + co[q]);
+                    const double2 tc = lds128(s1 + co[q]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int k = 2 * q + e;
+                        const bool isB = (ks >= 0 && k >= ks);
+                        const TRowCoef<DEGK> c = trow_coef<DEGK>(isB ? A.layB : A.layA);
+                        const double a_ = e ? tc.y : tc.x, d_ = e ? td.y : td.x;
+                        fl[2 * h + e] = wlam<DEGK, true>(c.K, isB ? A.sqB : A.sqA, a_ + d_) * (a_ - d_);
+                    }
+                }
+                tmem_st4(tm + tcol_flux(g), fl[0], fl[1], fl[2], fl[3]);
+            }
+            tmem_wait_st();
+        }
+        __syncwarp();
+        if (lane == 0 && NS <= nl + 1) issue_load((uint32_t)NS); // the slot of line j0 - 1 is free again
+
+        for (int L = 0; L < nl; ++L) {
+            const uint32_t q = qbase + (uint32_t)(L + 1);
+            const uint32_t qs = q % (uint32_t)NS, qu = (q + 1u) % (uint32_t)NS;
+            const uint32_t sc = wbase + qs * (uint32_t)SLOT; // line j   (centre)
+            const uint32_t su = wbase + qu * (uint32_t)SLOT; // line j+1 (up)
+            const int j = j0 + L;
+            const double ezm = __ldg(p.ezm + j), ezp = __ldg(p.ezp + j);
+            asm volatile("" : "+d"(fi0)); // keep the per-row geometry out of registers across lines
+            wait_seq((uint32_t)(L + 2));
+
+            // ---- the two r neighbours of the thread's 16 nodes at line j
+            double hl, hr;
+            {
+                const double2 v0 = lds128(sc + co[0]);
+                const double2 v7 = lds128(sc + co[7]);
+                hl = v0.x; hr = v7.y;
+            }
+            if (lane > 0) hl = lds64(sc + hlo);
+            else if (has_l) hl = lds64(halo_a + qs * 32u + 8u);
+            if (lane < 31) hr = lds64(sc + hro);
+            else if (has_r) hr = lds64(halo_a + qs * 32u + 16u);
+
+            // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 16 rows
+            A.sc = sc; A.su = su; A.hl = hl; A.hr = hr; A.fi0 = fi0; A.ezp = ezp; A.ezm = ezm;
+            const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, co) : tsweep16<DEGK, false>(A, co);
+            tmem_wait_st();
+            // the slot of line j - 1 has been stored (its TMA store was issued a whole sweep ago): refill it
+            if (lane == 0 && L >= 1 && L + NS <= nl + 1) { tma_wait_read0(); issue_load((uint32_t)(L + NS)); }
+
+            // ---- reduced row of this thread: a*y_{t-1} + y_t + c*y_{t+1} = d  (y = x of the last row)
+            double Pn = __shfl_down_sync(FULL, o.P, 1);
+            double Qn = __shfl_down_sync(FULL, o.Q, 1);
+            double Sn = __shfl_down_sync(FULL, o.S, 1);
+            if (lane == 31) { Pn = 0.0; Qn = 0.0; Sn = 0.0; }
+            Row3 row;
+            {
+                const double r = rcp_cubic(fma(-o.al, Sn, 1.0));
+                row.a = -o.gm * r;
+                row.c = -o.al * Pn * r;
+                row.d = fma(o.al, Qn, o.be) * r;
+            }
+            double y, u;
+            if constexpr (WL == 1) {
+                // the whole line is this warp: PCR over all 32 reduced rows
+                row = pcr_segment_rolled<32>(row, lane, 0, 31);
+                y = row.d;
+                u = __shfl_up_sync(FULL, y, 1);
+                if (lane == 0) u = 0.0;
+            } else {
+                // ---- level 2: PCR over lanes 0..30; lane 31 is the warp's separator
+                const Row3 rp = pcr_lanes_0_30_rolled(row, lane);
+                Row3 r30;
+                r30.a = __shfl_sync(FULL, rp.a, 30);
+                r30.c = __shfl_sync(FULL, rp.c, 30);
+                r30.d = __shfl_sync(FULL, rp.d, 30);
+                // publish what the separator solve needs from this warp (12 doubles) to every CTA of the
+                // line: asynchronous (distributed) shared-memory stores that complete on the receiver's
+                // mbarrier, so neither a barrier nor a release fence is needed
+                const uint32_t pubpar = lcount & 1u;
+                const uint32_t pbar = xbar_a + 8u * pubpar;
+                const uint32_t pub0 = pub_a + (uint32_t)((pubpar * LPB + grp) * WL * Cfg::PUB) * 8u;
+                if (wl == 0 && lane == 1) mbar_expect_tx(pbar, (uint32_t)(WL * Cfg::PUB * 8));
+                if (lane == 0 || lane == 31) {
+                    const uint32_t s6 = pub0 + (uint32_t)(wig * Cfg::PUB) * 8u + (lane == 31 ? 48u : 0u);
+                    const double v0 = lane == 31 ? o.al : o.P, v1 = lane == 31 ? o.be : o.Q, v2 = lane == 31 ? o.gm : o.S;
+                    const double v3 = lane == 31 ? r30.a : rp.a, v4 = lane == 31 ? r30.c : rp.c, v5 = lane == 31 ? r30.d : rp.d;
+#pragma unroll
+                    for (int rk = 0; rk < CL; ++rk) {
+                        const uint32_t ra = map_to_rank(s6, (uint32_t)rk), rb = map_to_rank(pbar, (uint32_t)rk);
+                        st_async_v2(ra, v0, v1, rb);
+                        st_async_v2(ra + 16, v2, v3, rb);
+                        st_async_v2(ra + 32, v4, v5, rb);
+                    }
+                }
+                while (!mbar_try_wait(pbar, (lcount >> 1) & 1u)) {}
+                // ---- level 3: every warp builds the WL separator rows and solves them (PCR, WL lanes)
+                double ys;
+                {
+                    const bool in3 = lane < WL;
+                    const int s = in3 ? lane : 0;
+                    const bool has_next = (s + 1 < WL);
+                    const int sn = has_next ? s + 1 : s;
+                    const uint32_t Da = pub0 + (uint32_t)(s * Cfg::PUB) * 8u;
+                    const uint32_t Dn = pub0 + (uint32_t)(sn * Cfg::PUB) * 8u;
+                    const double2 d3 = lds128(Da + 48), d4 = lds128(Da + 64), d5 = lds128(Da + 80);
+                    const double2 n0 = lds128(Dn), n1 = lds128(Dn + 16), n2 = lds128(Dn + 32);
+                    const double sal = d3.x, sbe = d3.y, sgm = d4.x;
+                    Row3 l30; l30.a = d4.y; l30.c = d5.x; l30.d = d5.y;
+                    Row3 nx; nx.a = nx.c = nx.d = 0.0;
+                    double Pw = 0.0, Qw = 0.0, Sw = 0.0;
+                    if (has_next) { Pw = n0.x; Qw = n0.y; Sw = n1.x; nx.a = n1.y; nx.c = n2.x; nx.d = n2.y; }
+                    Row3 me;
+                    const double r = rcp_cubic(fma(-sal, Sw, 1.0));
+                    me.a = -sgm * r;
+                    me.c = -sal * Pw * r;
+                    me.d = fma(sal, Qw, sbe) * r;
+                    Row3 s3 = pcr_combine(me, l30, true, nx, has_next);
+                    s3 = pcr_segment_rolled<WL>(s3, s, 0, WL - 1);
+                    ys = s3.d;
+                }
+                const double Vs = __shfl_sync(FULL, ys, wig);
+                double U = __shfl_sync(FULL, ys, (wig + WL - 1) % WL);
+                if (wig == 0) U = 0.0;
+                y = (lane == 31) ? Vs : fma(-rp.c, Vs, fma(-rp.a, U, rp.d));
+                u = __shfl_up_sync(FULL, y, 1);
+                if (lane == 0) u = U;
+            }
+            ++lcount;
+
+            // ---- back substitution (14) P:L150 with (alpha, beta, gamma) read back from tensor memory,
+            //      four rows at a time, the next group in flight; the new level replaces line j in its slot
+            double x[16];
+            x[15] = y;
+            {
+                TRaw8 c0, c1, c2, n0, n1, n2;
+                tmem_ld8(tm + tcol_coef(3, 0), c0);
+                tmem_ld8(tm + tcol_coef(3, 1), c1);
+                tmem_ld8(tm + tcol_coef(3, 2), c2);
+#pragma unroll
+                for (int g = 3; g >= 0; --g) {
+                    tmem_wait_ld3(c0, c1, c2);
+                    if (g > 0) {
+                        tmem_ld8(tm + tcol_coef(g > 0 ? g - 1 : 0, 0), n0);
+                        tmem_ld8(tm + tcol_coef(g > 0 ? g - 1 : 0, 1), n1);
+                        tmem_ld8(tm + tcol_coef(g > 0 ? g - 1 : 0, 2), n2);
+                    }
+                    // the group's twelve doubles: (al, be, gm) of rows 4g .. 4g+3
+                    double cf[12];
+#pragma unroll
+                    for (int n = 0; n < 4; ++n) { cf[n] = traw(c0, n); cf[4 + n] = traw(c1, n); cf[8 + n] = traw(c2, n); }
+#pragma unroll
+                    for (int r = 3; r >= 0; --r) {
+                        const int k = 4 * g + r;
+                        if (k < 15) x[k] = fma(cf[3 * r], x[k + 1], fma(cf[3 * r + 2], u, cf[3 * r + 1]));
+                    }
+                    if (g > 0) { c0 = n0; c1 = n1; c2 = n2; }
+                }
+            }
+#pragma unroll
+            for (int qq = 0; qq < 8; ++qq) sts128(sc + co[qq], x[2 * qq], x[2 * qq + 1]);
+            fence_proxy_async();
+            __syncwarp();
+
+            // ---- the warp's own TMA store of its 4 KB of the new level; Neumann z lines copy their
+            //      neighbour (reading G16)
+            if (lane == 0) {
+                const int Rg = (b * nz + j) * rpl + wig * 32;
+                tma_store_2d(&p.tm_st, 0, Rg, sc);
+                if (j == 1 && p.z_lo_neumann) tma_store_2d(&p.tm_st, 0, Rg - rpl, sc);
+                if (j == nz - 2 && p.z_hi_neumann) tma_store_2d(&p.tm_st, 0, Rg + rpl, sc);
+                tma_commit();
+            }
+
+            // ---- probes: T of the new level at (i_p, j_p)
+            if (p.probe_out != nullptr) {
+                for (int pq = 0; pq < p.nprobes; ++pq) {
+                    const ProbeSrc ps = p.probes[pq];
+                    if (ps.i < i0 || ps.i >= i0 + 16) continue;
+                    if (ps.is_static) {
+                        if (j == 1) p.probe_out[b * p.nprobes + pq] = p.Told[((size_t)b * nz + ps.j_store) * p.nr + ps.i];
+                    } else if (ps.j_src == j) {
+                        double v = 0.0;
+#pragma unroll
+                        for (int k = 0; k < 16; ++k)
+                            if (i0 + k == ps.i) v = x[k];
+                        p.probe_out[b * p.nprobes + pq] = v;
+                    }
+                }
+            }
+        }
+        if (lane == 0) tma_wait_read0(); // the next band's loads reuse the slots
+        __syncwarp();
+        qbase += (uint32_t)(nl + 2);
+    }
+    if (lane == 0) tma_wait_all0();
+    // every warp is done with its strip before warp 0 gives the tensor memory back
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(Cfg::TCOLS) : "memory");
+    if (CL > 1) { cluster_arrive(); cluster_wait(); }
+}
+
+} // namespace heat

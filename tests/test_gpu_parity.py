@@ -166,6 +166,7 @@ def test_wband_kernel_edge_cases(bd, case, monkeypatch):
     initial field, source with sub-steps, probes on boundary / interface / Dirichlet nodes,
     ragged band partition, 1..16 warps per line in clusters of 1, 2, 4 and 8 CTAs."""
     nr, nz, batch, poly, bcs, nw = case
+    monkeypatch.setenv("HEAT_KERNEL", "wband")   # the register version (tband takes precedence otherwise)
     monkeypatch.setenv("HEAT_WBAND_NW", str(nw))
     s = I.band_spec(nr + nz, nr=nr, nz=nz, batch=batch, bcs=bcs, poly_laws=poly, chunk=16)
     s = with_dt(bd, s, 0.8)
@@ -182,11 +183,64 @@ def test_wband_kernel_edge_cases(bd, case, monkeypatch):
     sim.close()
 
 
+TBAND_CASES = [
+    # nr, nz, batch, poly laws, bcs, HEAT_TBAND_NW
+    (512, 24, 3, False, None, 4),              # one warp per line, four lines per CTA
+    (512, 9, 5, True, BC_SETS[1], 4),          # ragged last round, Neumann z_lo
+    (1024, 21, 2, False, BC_SETS[2], 4),       # two warps per line, Dirichlet r boundaries
+    (2048, 19, 1, True, BC_SETS[3], 4),        # a CTA per line
+    (4096, 12, 1, False, None, 4),             # cluster of 2 CTAs per line
+    (8192, 7, 1, False, BC_SETS[1], 4),        # cluster of 4, Neumann z_lo
+    (8192, 6, 2, True, None, 8),               # cluster of 2 CTAs of 8 warps
+    (8192, 9, 1, False, BC_SETS[3], 16),       # one CTA of 16 warps per line, no cluster
+]
+
+
+@pytest.mark.parametrize("case", TBAND_CASES, ids=lambda c: f"nr{c[0]}-nz{c[1]}-b{c[2]}-{'poly' if c[3] else 'pow'}-nw{c[5]}")
+def test_tband_kernel_edge_cases(bd, case, monkeypatch):
+    """The tensor-memory band kernel (the one bench.py times) on the band_spec problems: interface
+    nodes at the first / last / middle row of a thread's chunk, square root, power and degree-4
+    polynomial laws side by side in one warp, every BC kind, non-uniform z, random initial field,
+    source with sub-steps, probes on boundary / interface / Dirichlet nodes, ragged band
+    partition, 1..16 warps per line in clusters of 1, 2 and 4 CTAs."""
+    nr, nz, batch, poly, bcs, nw = case
+    monkeypatch.setenv("HEAT_TBAND_NW", str(nw))
+    s = I.band_spec(nr + nz, nr=nr, nz=nz, batch=batch, bcs=bcs, poly_laws=poly, chunk=16)
+    s = with_dt(bd, s, 0.8)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp" if nr * nz > 30000 else "double")
+    assert sim.kernel_name.startswith(f"tband<WL={nr // 512},NW={nw},"), sim.kernel_name
+    for n in (1, 6, 13):
+        sim.step(n)
+        orc.step(n)
+        compare(sim, orc)
+    pg, dropped = sim.probes()
+    po = orc.probes()
+    assert dropped == 0 and pg.shape == po.shape
+    assert np.max(np.abs(pg - po)) <= TOL
+    sim.close()
+
+
+def test_tband_kernel_band_length_does_not_change_the_result(bd, monkeypatch):
+    """The partition of the lines into bands is a scheduling choice: the field is bitwise the
+    same for bands of 1, 3 and all lines."""
+    s = with_dt(bd, I.band_spec(7, nr=1024, nz=20, batch=2, chunk=16), 0.8)
+    out = []
+    for bl in ("1", "3", "18"):
+        monkeypatch.setenv("HEAT_BAND_LINES", bl)
+        sim = bd.HeatSim(s)
+        assert sim.kernel_name.startswith("tband<"), sim.kernel_name
+        sim.step(9)
+        out.append(sim.fields())
+        sim.close()
+    assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
+
+
 def test_wband_kernel_band_length_does_not_change_the_result(bd, monkeypatch):
     """The partition of the lines into bands is a scheduling choice: the field is bitwise the
     same for bands of 1, 3 and all lines."""
     s = with_dt(bd, I.band_spec(7, nr=1024, nz=20, batch=2, chunk=16), 0.8)
     out = []
+    monkeypatch.setenv("HEAT_KERNEL", "wband")
     for bl in ("1", "3", "18"):
         monkeypatch.setenv("HEAT_BAND_LINES", bl)
         sim = bd.HeatSim(s)
