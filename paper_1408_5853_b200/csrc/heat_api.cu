@@ -941,6 +941,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         // tcgen05.alloc although 16 / NW are resident; registers (128) and shared memory (<= 52 KB per
         // four warps) allow them, see the static_asserts in heat_tband_kernel.cuh.)
         if (tbv) max_clusters = prop.multiProcessorCount * (warps_per_sm / wNW) / wCL;
+        if (const char *em = getenv("HEAT_MAX_CLUSTERS")) max_clusters = std::max(1, atoi(em));
         if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / wCL);
         // bands: every line group (LPB per CTA) walks BL consecutive lines of one batch member;
         // choose the band count per member that minimises rounds * (BL + prologue)
@@ -1000,6 +1001,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         wp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
         wp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
         wp.rpl = nr / 16; wp.BL = best_BL; wp.bands_per_member = bpm; wp.total_bands = (int)bands;
+        wp.stagger = 0;
+        if (const char *es = getenv("HEAT_STAGGER")) wp.stagger = atoi(es);
     }
 
     KParams &k = c->kp;

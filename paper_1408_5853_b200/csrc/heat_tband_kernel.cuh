@@ -38,7 +38,9 @@ struct TBandCfg {
     static constexpr int OFF_PUB = OFF_HALO + NW * NS * 32;           // [2][LPB][WL][PUB]
     static constexpr int OFF_FBAR = OFF_PUB + 2 * LPB * WL * PUB * 8; // [NW][NS] load barriers
     static constexpr int OFF_XBAR = OFF_FBAR + NW * NS * 8;           // [LPB][2] exchange barriers
-    static constexpr int OFF_TMEM = OFF_XBAR + LPB * 2 * 8;           // tensor-memory base address
+    static constexpr int OFF_YBAR = OFF_XBAR + LPB * 2 * 8;           // [LPB][2] separator-solution barriers
+    static constexpr int OFF_YSEP = OFF_YBAR + LPB * 2 * 8;           // [2][LPB][WL] separator values
+    static constexpr int OFF_TMEM = OFF_YSEP + 2 * LPB * WL * 8;      // tensor-memory base address
     static constexpr int OFF_LAY = OFF_TMEM + 16;
     static constexpr size_t smem_bytes(int nlayers) { return 1024 + (size_t)OFF_LAY + sizeof(WLayer) * (size_t)nlayers; }
 };
@@ -136,97 +138,134 @@ __device__ __forceinline__ TRowCoef<DEGK> trow_coef(uint32_t a)
     return c;
 }
 
-// Level 1 for one thread: rows (13) P:L140-145 assembled and pushed through the sweep (12)
-// P:L133-136, sixteen rows in four groups of four; (alpha, beta, gamma) and the new face fluxes of a
-// group go to tensor memory, the prefix products for the reduced row are carried along.  Special
-// rows as in wsweep16 (heat_wband_kernel.cuh): no branch inside the row loop.
+// Four consecutive rows (13) P:L140-145 of one thread, assembled and pushed through the sweep (12)
+// P:L133-136.  g = group (rows 4g .. 4g+3), runtime.
+// GEN = false: regular rows of the layer whose coefficients sit in registers (c): the plain, fast body.
+// GEN = true : the group may hold an interface row (18)-(20) P:L176-192 (row ks: the two face
+//              coefficients become lam*_A, lam*_B, capacity and right-hand side vanish, and from it on
+//              the rows are layer B's, G14) or an r-boundary row (15)-(17) P:L158-174 (a Neumann row
+//              is an ordinary row with a zero face and zero capacity, a Dirichlet row is a select);
+//              coefficients are read row by row from the shared table.  Still no branch per row.
+// The caller picks the body per warp and group (warp-uniform), so the common case runs the plain body
+// and the instruction cache holds four rows of each kind instead of sixteen.
+template <int DEGK, bool SQ, bool GEN>
+__device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, const WCoef<DEGK> &c, SweepState &st, TSweepOut &o,
+                                       double2 &tl, double lamA_if, double lamB_if)
+{
+    TRaw8 fraw;
+    tmem_ld8(A.tm + 96u + 8u * (uint32_t)g, fraw); // the four lower face fluxes of the group
+    const uint32_t q0 = 2u * (uint32_t)g;
+    const uint32_t o0 = A.rowo + (((q0) ^ A.sw) << 4), o1 = A.rowo + (((q0 + 1u) ^ A.sw) << 4);
+    const uint32_t o2 = A.rowo + (((q0 + 2u) & 7u) ^ A.sw) * 16u;
+    const double2 t1 = lds128(A.sc + o1);
+    double2 t2 = lds128(A.sc + o2); // rows 4g+4, 4g+5 (the next group's first pair); beyond the chunk: hr
+    if (g == 3) t2 = make_double2(A.hr, A.hr);
+    const double2 u0 = lds128(A.su + o0), u1 = lds128(A.su + o1);
+    const double fig = A.fi0 + (double)(4 * g);
+    const bool lastg = (g == 3);
+    const uint32_t ksw = (GEN && A.ks >= 0) ? (uint32_t)A.ks : 99u;
+    tmem_wait_ld(fraw);
+    double fD[4], cf[12], fu[4];
+#pragma unroll
+    for (int n = 0; n < 4; ++n) fD[n] = traw(fraw, n);
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const double T = (r == 0) ? tl.x : (r == 1) ? tl.y : (r == 2) ? t1.x : t1.y;
+        const double Tr = (r == 0) ? tl.y : (r == 1) ? t1.x : (r == 2) ? t1.y : t2.x;
+        const double Tu = (r == 0) ? u0.x : (r == 1) ? u0.y : (r == 2) ? u1.x : u1.y;
+        const uint32_t k = 4u * (uint32_t)g + (uint32_t)r;
+        const double fi = fig + (double)r;
+        double cfR, w, f, alk;
+        if (!GEN) {
+            wrow2<DEGK, SQ>(c.K, c.Ct, c.qs, c.sq, T, Tr, Tu, fD[r], fi, fi, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
+            sweep_row(st, cfR, w, f, alk);
+        } else {
+            const bool isB = (k >= ksw), isif = (k == ksw);
+            const TRowCoef<DEGK> cr = trow_coef<DEGK>(isB ? A.layB : A.layA);
+            const double qs = isB ? A.qsB : A.qsA;
+            const bool sq = isB ? A.sqB : A.sqA;
+            double fie = fi;
+            if (r == 3) fie = lastg ? A.fie15 : fie;
+            fie = isif ? 0.0 : fie;
+            wrow2<DEGK, SQ>(cr.K, cr.Ct, qs, sq, T, Tr, Tu, fD[r], fi, fie, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
+            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
+            double cfL_use = isif ? lamA_if : st.cfL;
+            double cfR_use = isif ? lamB_if : cfR;
+            if (r == 3) { // row 15: r_out row (15),(17): x_N = x_{N-1} (fie15 = 0, no right face) or x_N = value
+                cfR_use = (lastg && A.last) ? 0.0 : cfR_use;
+                cfL_use = (lastg && A.dout) ? 0.0 : cfL_use;
+                w = (lastg && A.dout) ? 1.0 : w;
+                f = (lastg && A.dout) ? A.rout_f : f;
+            }
+            st.cfL = cfL_use;
+            sweep_row(st, cfR_use, w, f, alk);
+            st.cfL = cfR; // face i + 1/2 as the next regular row sees it
+            if (r == 0) { // row 0: r_in row (15),(16): alpha_0 = 1 exactly (T^_0 = T^_1 bitwise); Dirichlet: x_0 = value
+                const bool g0_ = (g == 0);
+                alk = (g0_ && A.nin) ? 1.0 : alk;
+                alk = (g0_ && A.din) ? 0.0 : alk;
+                st.om = (g0_ && A.din) ? 1.0 : st.om;
+                st.be = (g0_ && A.din) ? A.rin_be : st.be;
+                st.gm = (g0_ && A.din) ? 0.0 : st.gm;
+            }
+        }
+        cf[3 * r] = alk; cf[3 * r + 1] = st.be; cf[3 * r + 2] = st.gm;
+        // x_0 = P x_{k+1} + Q + S u (rows 0 .. 14)
+        const double Qn = fma(o.P, st.be, o.Q), Sn = fma(o.P, st.gm, o.S), Pn = o.P * alk;
+        if (r < 3) { o.Q = Qn; o.S = Sn; o.P = Pn; }
+        else { o.Q = lastg ? o.Q : Qn; o.S = lastg ? o.S : Sn; o.P = lastg ? o.P : Pn; }
+    }
+    tl = t2;
+    const uint32_t tc = A.tm + 24u * (uint32_t)g;
+    tmem_st4(tc, cf[0], cf[1], cf[2], cf[3]);
+    tmem_st4(tc + 8u, cf[4], cf[5], cf[6], cf[7]);
+    tmem_st4(tc + 16u, cf[8], cf[9], cf[10], cf[11]);
+    tmem_st4(A.tm + 96u + 8u * (uint32_t)g, fu[0], fu[1], fu[2], fu[3]);
+    o.al = cf[9]; o.be = cf[10]; o.gm = cf[11];
+}
+
+// Level 1 for one thread: the sixteen rows in four groups of four (a rolled loop); (alpha, beta,
+// gamma) and the new face fluxes of a group go to tensor memory, the prefix products for the reduced
+// row are carried along.  genmask: bit g set = group g of this warp needs the general body.
 template <int DEGK, bool SQ>
-__device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, const uint32_t (&co)[8])
+__device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, WCoef<DEGK> &c, uint32_t genmask)
 {
     SweepState st;
     st.om = 1.0; st.be = 0.0; st.gm = 1.0;
     TSweepOut o;
     o.P = 1.0; o.Q = 0.0; o.S = 0.0;
-    // interface node: lam*_A, lam*_B at T_{i*,j} of the old level
+    // interface node: lam*_A, lam*_B at T_{i*,j} of the old level; the thread that holds one
+    // starts every line with layer A's coefficients
     double lamA_if = 0.0, lamB_if = 0.0;
     if (A.ks >= 0) {
         const double Tk = lds64(A.sc + A.rowo + ((((uint32_t)A.ks >> 1) ^ A.sw) << 4) + (((uint32_t)A.ks & 1u) << 3));
         const TRowCoef<DEGK> ca = trow_coef<DEGK>(A.layA), cb = trow_coef<DEGK>(A.layB);
         lamA_if = wlam<DEGK, true>(ca.K, A.sqA, Tk + Tk);
         lamB_if = wlam<DEGK, true>(cb.K, A.sqB, Tk + Tk);
-    }
-    const uint32_t ksw = (A.ks >= 0) ? (uint32_t)A.ks : 99u;
-    TRaw8 fraw;
-    tmem_ld8(A.tm + tcol_flux(0), fraw);
-    double2 tl = lds128(A.sc + co[0]);
-    {
-        const TRowCoef<DEGK> c0 = trow_coef<DEGK>(A.layA);
-        st.cfL = wlam<DEGK, SQ>(c0.K, A.sqA, A.hl + tl.x) * A.gl0; // face i0 - 1/2
-    }
 #pragma unroll
+        for (int n = 0; n <= DEGK; ++n) c.K[n] = ca.K[n];
+#pragma unroll
+        for (int n = 0; n < 4; ++n) c.Ct[n] = ca.Ct[n];
+        c.qs = A.qsA; c.sq = A.sqA;
+    }
+    double2 tl = lds128(A.sc + A.rowo + (A.sw << 4));
+    st.cfL = wlam<DEGK, SQ>(c.K, c.sq, A.hl + tl.x) * A.gl0; // face i0 - 1/2
+#pragma unroll 1
     for (int g = 0; g < 4; ++g) {
-        tmem_wait_ld(fraw);
-        double fD[4];
+        if (!((genmask >> g) & 1u)) {
+            tgroup<DEGK, SQ, false>(A, g, c, st, o, tl, lamA_if, lamB_if);
+        } else {
+            tgroup<DEGK, SQ, true>(A, g, c, st, o, tl, lamA_if, lamB_if);
+            // behind its interface row the thread is in layer B
+            if (A.ks >= 0 && (A.ks >> 2) == g) {
+                const TRowCoef<DEGK> cb = trow_coef<DEGK>(A.layB);
 #pragma unroll
-        for (int n = 0; n < 4; ++n) fD[n] = traw(fraw, n);
-        if (g < 3) tmem_ld8(A.tm + tcol_flux(g < 3 ? g + 1 : 3), fraw);
-        double cf[12], fu[4];
-        double2 tn, tu;
+                for (int n = 0; n <= DEGK; ++n) c.K[n] = cb.K[n];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int k = 4 * g + r, qq = k >> 1, e = k & 1;
-            double T, Tr, Tu;
-            if (e == 0) { // tl holds (T_k, T_{k+1})
-                tu = lds128(A.su + co[qq]);
-                T = tl.x; Tr = tl.y; Tu = tu.x;
-            } else {
-                if (qq < 7) tn = lds128(A.sc + co[qq < 7 ? qq + 1 : 7]);
-                else tn = make_double2(A.hr, A.hr);
-                T = tl.y; Tr = tn.x; Tu = tu.y;
+                for (int n = 0; n < 4; ++n) c.Ct[n] = cb.Ct[n];
+                c.qs = A.qsB; c.sq = A.sqB;
             }
-            const bool isB = ((uint32_t)k >= ksw);
-            const bool isif = ((uint32_t)k == ksw);
-            const TRowCoef<DEGK> c = trow_coef<DEGK>(isB ? A.layB : A.layA);
-            const double qs = isB ? A.qsB : A.qsA;
-            const bool sq = isB ? A.sqB : A.sqA;
-            const double fi = A.fi0 + (double)k;
-            double fie = (k == 15) ? A.fie15 : fi;
-            fie = isif ? 0.0 : fie;
-            double cfR, w, f;
-            wrow2<DEGK, SQ>(c.K, c.Ct, qs, sq, T, Tr, Tu, fD[r], fi, fie, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
-            // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
-            double cfL_use = isif ? lamA_if : st.cfL;
-            double cfR_use = isif ? lamB_if : cfR;
-            if (k == 15) { // r_out row (15),(17): x_N = x_{N-1} (fie15 = 0, no right face) or x_N = value
-                cfR_use = A.last ? 0.0 : cfR_use;
-                cfL_use = A.dout ? 0.0 : cfL_use;
-                w = A.dout ? 1.0 : w;
-                f = A.dout ? A.rout_f : f;
-            }
-            st.cfL = cfL_use;
-            double alk;
-            sweep_row(st, cfR_use, w, f, alk);
-            st.cfL = cfR; // face i + 1/2 as the next regular row sees it
-            if (k == 0) { // r_in row (15),(16): alpha_0 = 1 exactly (T^_0 = T^_1 bitwise); Dirichlet: x_0 = value
-                alk = A.nin ? 1.0 : alk;
-                alk = A.din ? 0.0 : alk;
-                st.om = A.din ? 1.0 : st.om;
-                st.be = A.din ? A.rin_be : st.be;
-                st.gm = A.din ? 0.0 : st.gm;
-            }
-            cf[3 * r] = alk; cf[3 * r + 1] = st.be; cf[3 * r + 2] = st.gm;
-            if (k < 15) { // x_0 = P x_{k+1} + Q + S u
-                o.Q = fma(o.P, st.be, o.Q);
-                o.S = fma(o.P, st.gm, o.S);
-                o.P = o.P * alk;
-            }
-            if (e == 1) tl = tn;
         }
-        tmem_st4(A.tm + tcol_coef(g, 0), cf[0], cf[1], cf[2], cf[3]);
-        tmem_st4(A.tm + tcol_coef(g, 1), cf[4], cf[5], cf[6], cf[7]);
-        tmem_st4(A.tm + tcol_coef(g, 2), cf[8], cf[9], cf[10], cf[11]);
-        tmem_st4(A.tm + tcol_flux(g), fu[0], fu[1], fu[2], fu[3]);
-        if (g == 3) { o.al = cf[9]; o.be = cf[10]; o.gm = cf[11]; }
     }
     return o;
 }
@@ -259,6 +298,8 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
     const uint32_t halo_a = sbase + Cfg::OFF_HALO + (uint32_t)(warp * NS) * 32u;
     const uint32_t fbar_a = sbase + Cfg::OFF_FBAR + (uint32_t)(warp * NS) * 8u;
     const uint32_t xbar_a = sbase + Cfg::OFF_XBAR + (uint32_t)grp * 16u;
+    const uint32_t ybar_a = sbase + Cfg::OFF_YBAR + (uint32_t)grp * 16u;
+    const uint32_t ysep_a = sbase + Cfg::OFF_YSEP;
     const uint32_t pub_a = sbase + Cfg::OFF_PUB;
     // byte offsets of the thread's eight 16-byte chunks inside a SWIZZLE_128B slot, and of its two
     // r neighbours (last node of the row above, first node of the row below)
@@ -288,6 +329,8 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
         for (int s = 0; s < NW * NS; ++s) mbar_init(sbase + Cfg::OFF_FBAR + 8u * s, 1);
 #pragma unroll 1
         for (int s = 0; s < LPB * 2; ++s) mbar_init(sbase + Cfg::OFF_XBAR + 8u * s, 1);
+#pragma unroll 1
+        for (int s = 0; s < LPB * 2; ++s) mbar_init(sbase + Cfg::OFF_YBAR + 8u * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -311,6 +354,13 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
     double fi0 = (double)i0;
     uint32_t qbase = 0;  // load sequence number of line offset -1 of this band
     uint32_t lcount = 0; // lines done (phase of the exchange barriers)
+
+    // CTAs that share an SM work on different lines; start them out of phase so that one sweeps (FP64
+    // pipe) while the other sits in its reduced system (latency)
+    if (p.stagger > 0 && (cluster_id & 1)) {
+        const long long t0 = clock64();
+        while (clock64() - t0 < (long long)p.stagger) {}
+    }
 
     for (int round = 0;; ++round) {
         const int band = (round * nclusters + cluster_id) * LPB + grp;
@@ -355,6 +405,10 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
         A.ks = ks; A.din = first && !rin_neu; A.dout = last && !rout_neu; A.nin = first && rin_neu; A.last = last;
         A.rin_be = p.rin_be; A.rout_f = p.rout_f;
         const bool anysq = __any_sync(FULL, A.sqA || (ks >= 0 && A.sqB));
+        WCoef<DEGK> c = wload_coef<DEGK>(lay[la], q0b); // the thread's current layer (A at the start of a line)
+        // groups of four rows that need the general body: the one with the interface row, the first
+        // group of the first chunk and the last group of the last chunk of the line
+        const uint32_t genmask = __reduce_or_sync(FULL, (ks >= 0 ? (1u << (ks >> 2)) : 0u) | (first ? 1u : 0u) | (last ? 8u : 0u));
 
         if (lane == 0) {
             const uint32_t npre = (uint32_t)min(NS, nl + 2);
@@ -415,7 +469,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
 
             // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 16 rows
             A.sc = sc; A.su = su; A.hl = hl; A.hr = hr; A.fi0 = fi0; A.ezp = ezp; A.ezm = ezm;
-            const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, co) : tsweep16<DEGK, false>(A, co);
+            const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, c, genmask) : tsweep16<DEGK, false>(A, c, genmask);
             tmem_wait_st();
             // the slot of line j - 1 has been stored (its TMA store was issued a whole sweep ago): refill it
             if (lane == 0 && L >= 1 && L + NS <= nl + 1) { tma_wait_read0(); issue_load((uint32_t)(L + NS)); }
@@ -452,7 +506,10 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                 const uint32_t pubpar = lcount & 1u;
                 const uint32_t pbar = xbar_a + 8u * pubpar;
                 const uint32_t pub0 = pub_a + (uint32_t)((pubpar * LPB + grp) * WL * Cfg::PUB) * 8u;
-                if (wl == 0 && lane == 1) mbar_expect_tx(pbar, (uint32_t)(WL * Cfg::PUB * 8));
+                // one warp of the CTA (in turn) solves the separator rows for all the others
+                const bool duty = ((uint32_t)wl == lcount % (uint32_t)WPL);
+                const uint32_t ysl = ysep_a + (uint32_t)((pubpar * LPB + grp) * WL) * 8u;
+                if (duty && lane == 1) mbar_expect_tx(pbar, (uint32_t)(WL * Cfg::PUB * 8));
                 if (lane == 0 || lane == 31) {
                     const uint32_t s6 = pub0 + (uint32_t)(wig * Cfg::PUB) * 8u + (lane == 31 ? 48u : 0u);
                     const double v0 = lane == 31 ? o.al : o.P, v1 = lane == 31 ? o.be : o.Q, v2 = lane == 31 ? o.gm : o.S;
@@ -465,10 +522,10 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                         st_async_v2(ra + 32, v4, v5, rb);
                     }
                 }
-                while (!mbar_try_wait(pbar, (lcount >> 1) & 1u)) {}
-                // ---- level 3: every warp builds the WL separator rows and solves them (PCR, WL lanes)
-                double ys;
-                {
+                double Vs, U;
+                if (duty) {
+                    while (!mbar_try_wait(pbar, (lcount >> 1) & 1u)) {}
+                    // ---- level 3: build the WL separator rows and solve them (PCR over WL lanes)
                     const bool in3 = lane < WL;
                     const int s = in3 ? lane : 0;
                     const bool has_next = (s + 1 < WL);
@@ -489,10 +546,16 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                     me.d = fma(sal, Qw, sbe) * r;
                     Row3 s3 = pcr_combine(me, l30, true, nx, has_next);
                     s3 = pcr_segment_rolled<WL>(s3, s, 0, WL - 1);
-                    ys = s3.d;
+                    if (in3) sts64(ysl + 8u * (uint32_t)lane, s3.d);
+                    __syncwarp();
+                    if (lane == 0) asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(ybar_a + 8u * pubpar) : "memory");
+                    Vs = __shfl_sync(FULL, s3.d, wig);
+                    U = __shfl_sync(FULL, s3.d, (wig + WL - 1) % WL);
+                } else {
+                    while (!mbar_try_wait(ybar_a + 8u * pubpar, (lcount >> 1) & 1u)) {}
+                    Vs = lds64(ysl + 8u * (uint32_t)wig);
+                    U = lds64(ysl + 8u * (uint32_t)((wig + WL - 1) % WL));
                 }
-                const double Vs = __shfl_sync(FULL, ys, wig);
-                double U = __shfl_sync(FULL, ys, (wig + WL - 1) % WL);
                 if (wig == 0) U = 0.0;
                 y = (lane == 31) ? Vs : fma(-rp.c, Vs, fma(-rp.a, U, rp.d));
                 u = __shfl_up_sync(FULL, y, 1);
@@ -501,36 +564,29 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             ++lcount;
 
             // ---- back substitution (14) P:L150 with (alpha, beta, gamma) read back from tensor memory,
-            //      four rows at a time, the next group in flight; the new level replaces line j in its slot
-            double x[16];
-            x[15] = y;
-            {
-                TRaw8 c0, c1, c2, n0, n1, n2;
-                tmem_ld8(tm + tcol_coef(3, 0), c0);
-                tmem_ld8(tm + tcol_coef(3, 1), c1);
-                tmem_ld8(tm + tcol_coef(3, 2), c2);
+            //      eight rows per wait; the new level replaces line j in its slot
+            double xn = y; // x_{k+1}
 #pragma unroll
-                for (int g = 3; g >= 0; --g) {
-                    tmem_wait_ld3(c0, c1, c2);
-                    if (g > 0) {
-                        tmem_ld8(tm + tcol_coef(g > 0 ? g - 1 : 0, 0), n0);
-                        tmem_ld8(tm + tcol_coef(g > 0 ? g - 1 : 0, 1), n1);
-                        tmem_ld8(tm + tcol_coef(g > 0 ? g - 1 : 0, 2), n2);
-                    }
-                    // the group's twelve doubles: (al, be, gm) of rows 4g .. 4g+3
-                    double cf[12];
+            for (int hh = 1; hh >= 0; --hh) {
+                TRaw8 cr[6];
 #pragma unroll
-                    for (int n = 0; n < 4; ++n) { cf[n] = traw(c0, n); cf[4 + n] = traw(c1, n); cf[8 + n] = traw(c2, n); }
+                for (int n = 0; n < 6; ++n) tmem_ld8(tm + (uint32_t)(48 * hh + 8 * n), cr[n]);
+                tmem_wait_ld3(cr[0], cr[1], cr[2]);
+                tmem_wait_ld3(cr[3], cr[4], cr[5]);
+                double xs[8];
 #pragma unroll
-                    for (int r = 3; r >= 0; --r) {
-                        const int k = 4 * g + r;
-                        if (k < 15) x[k] = fma(cf[3 * r], x[k + 1], fma(cf[3 * r + 2], u, cf[3 * r + 1]));
-                    }
-                    if (g > 0) { c0 = n0; c1 = n1; c2 = n2; }
+                for (int r = 7; r >= 0; --r) {
+                    // row k = 8 hh + r: its (al, be, gm) are doubles 3r, 3r+1, 3r+2 of the 24 loaded
+                    const int k = 8 * hh + r;
+                    const double a_ = traw(cr[(3 * r) >> 2], (3 * r) & 3);
+                    const double b_ = traw(cr[(3 * r + 1) >> 2], (3 * r + 1) & 3);
+                    const double g_ = traw(cr[(3 * r + 2) >> 2], (3 * r + 2) & 3);
+                    xs[r] = (k == 15) ? y : fma(a_, xn, fma(g_, u, b_));
+                    xn = xs[r];
                 }
-            }
 #pragma unroll
-            for (int qq = 0; qq < 8; ++qq) sts128(sc + co[qq], x[2 * qq], x[2 * qq + 1]);
+                for (int q2 = 0; q2 < 4; ++q2) sts128(sc + co[4 * hh + q2], xs[2 * q2], xs[2 * q2 + 1]);
+            }
             fence_proxy_async();
             __syncwarp();
 
@@ -552,11 +608,8 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                     if (ps.is_static) {
                         if (j == 1) p.probe_out[b * p.nprobes + pq] = p.Told[((size_t)b * nz + ps.j_store) * p.nr + ps.i];
                     } else if (ps.j_src == j) {
-                        double v = 0.0;
-#pragma unroll
-                        for (int k = 0; k < 16; ++k)
-                            if (i0 + k == ps.i) v = x[k];
-                        p.probe_out[b * p.nprobes + pq] = v;
+                        const uint32_t kk = (uint32_t)(ps.i - i0); // the value just written into the slot
+                        p.probe_out[b * p.nprobes + pq] = lds64(sc + (uint32_t)lane * 128u + ((((kk >> 1) ^ ((uint32_t)lane & 7u))) << 4) + ((kk & 1u) << 3));
                     }
                 }
             }
