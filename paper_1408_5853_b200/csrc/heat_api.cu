@@ -332,7 +332,8 @@ const WBandVariant *plan_wband(const heat_desc *d, std::vector<PLayer> *players,
     // the register version
     const char *ek = getenv("HEAT_KERNEL");
     if (tband && !(ek && strcmp(ek, "wband") == 0)) {
-        int TNW = 4;
+        // default: a whole line per CTA where that needs no cluster (nr = 8192: 16 warps, 4096: 8 warps)
+        int TNW = WL >= 16 ? 16 : WL >= 8 ? 8 : 4;
         if (const char *e = getenv("HEAT_TBAND_NW")) TNW = atoi(e);
         const TBandVariant *ttab = DEGK == 2 ? k_tband_variants2 : k_tband_variants4;
         const int nttab = DEGK == 2 ? k_ntband_variants2 : k_ntband_variants4;
@@ -940,8 +941,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         // fit.  (The occupancy query reports a single CTA per SM for a kernel that executes
         // tcgen05.alloc although 16 / NW are resident; registers (128) and shared memory (<= 52 KB per
         // four warps) allow them, see the static_asserts in heat_tband_kernel.cuh.)
-        if (tbv) max_clusters = prop.multiProcessorCount * (warps_per_sm / wNW) / wCL;
-        if (const char *em = getenv("HEAT_MAX_CLUSTERS")) max_clusters = std::max(1, atoi(em));
+        // For a cluster the query's answer (clusters at one CTA per SM) is scaled by the CTAs per SM.
+        if (tbv) max_clusters = (wCL == 1) ? prop.multiProcessorCount * (warps_per_sm / wNW) : max_clusters * (warps_per_sm / wNW);
         if (occ_cap_env > 0) max_clusters = std::min(max_clusters, prop.multiProcessorCount * occ_cap_env / wCL);
         // bands: every line group (LPB per CTA) walks BL consecutive lines of one batch member;
         // choose the band count per member that minimises rounds * (BL + prologue)
@@ -1001,8 +1002,6 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         wp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
         wp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
         wp.rpl = nr / 16; wp.BL = best_BL; wp.bands_per_member = bpm; wp.total_bands = (int)bands;
-        wp.stagger = 0;
-        if (const char *es = getenv("HEAT_STAGGER")) wp.stagger = atoi(es);
     }
 
     KParams &k = c->kp;

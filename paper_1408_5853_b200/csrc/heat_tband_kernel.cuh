@@ -357,11 +357,6 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
 
     // CTAs that share an SM work on different lines; start them out of phase so that one sweeps (FP64
     // pipe) while the other sits in its reduced system (latency)
-    if (p.stagger > 0 && (cluster_id & 1)) {
-        const long long t0 = clock64();
-        while (clock64() - t0 < (long long)p.stagger) {}
-    }
-
     for (int round = 0;; ++round) {
         const int band = (round * nclusters + cluster_id) * LPB + grp;
         if (band >= p.total_bands) break; // uniform over the warps of a line

@@ -294,3 +294,100 @@ def band_spec(seed, nr=512, nz=24, nlayers=4, batch=1, bcs=None, source=True, po
     s["probes"] = [(nr - 1, nz // 2), (0, 1), (int(np.flatnonzero(np.diff(segs[0].astype(int)))[0]) + 1, nz - 2), (17, 0)]
     s["probe_every"] = 2
     return s
+
+
+# ---------------------------------------------------------------- the paper's own device
+
+# Fit coefficients of Tables 2 and 3, units J/(g K), W/(cm K), g/cm^3, cm, K, as
+# printed and read in DESCENDING powers (reading G11: only then lambda_3 == 1e-3 as P:L276 says and
+# every lambda_m is positive on 4.2-60 K).  tests/golden/paper_tables_2_3.txt holds the same numbers
+# with their citations; tests/test_inputs.py checks the two against each other.
+PAPER_CV_DESC = {   # a3 a2 a1 a0
+    0: (0.0, 4.541e-4, -3.821e-3, 1e-2),
+    1: (-6.514e-7, 1.057e-4, 2.366e-2, -6.619e-3),
+    2: (-8.199e-7, 2.328e-5, -1.245e-4, 2.169e-4),
+    3: (0.0, 0.0, 2.35e-2, 2.0e-2),
+}
+PAPER_LAM_DESC = {  # b4 b3 b2 b1 b0
+    0: (7.029e-7, -9.317e-5, 2.306e-3, 1.166e-1, -1.139e-1),
+    1: (0.0, -2.523e-7, 2.038e-5, -1.248e-4, 6.77e-3),
+    2: (0.0, 3.03e-9, -6.369e-7, 1.05e-4, -2.729e-4),
+    3: (0.0, 0.0, 0.0, 0.0, 1e-3),
+}
+PAPER_RHO = (8.92, 2.0, 2.0, 2.5)
+# The printed graphite row (m = 2) has c_V < 0 above 22 K although the paper heats graphite past
+# 40 K (reading G11): a_3 = -8.199e-7 is taken as a misprint of -8.199e-9 (c_V(60 K) = 0.075 J/(g K)).
+# This is OUR substitution, not the paper's number; heat_create rejects the printed row.
+PAPER_GRAPHITE_A3_SUBSTITUTE = -8.199e-9
+PAPER_RADII_CM = (0.12, 0.125, 0.13, 0.1301)   # r_0, r_1, r_2, r_max
+PAPER_ZMAX_CM = 5.0                            # P:L300 (z_0 = 4 cm, reading G10, is not needed on a rectangle)
+PAPER_I0_A, PAPER_CHI0 = 0.363, 1.8            # I_0 P:L278; chi(T) = 1.8 / sqrt(T) Ohm cm, (25) P:L274
+PAPER_T0, PAPER_TCRIT = 4.2, 42.2
+
+
+def paper_layers(printed_graphite=False):
+    out = []
+    for m in range(4):
+        a = list(PAPER_CV_DESC[m])
+        if m == 2 and not printed_graphite:
+            a[0] = PAPER_GRAPHITE_A3_SUBSTITUTE
+        out.append(layer(poly(PAPER_LAM_DESC[m][::-1]), poly(a[::-1]), PAPER_RHO[m], is_heater=(m == 2),
+                         src_shape=power(1.0, -0.5, 1.0)))   # chi(T) ~ T^-1/2, (25)
+    return out
+
+
+def paper_radial_nodes(nr=631):
+    """The paper gives N = 631 but not the node distribution, only that the radial step must be
+    at least an order of magnitude below the layer thicknesses.  OUR recipe: with
+    u = (nr - 1) / 63 segments per unit, the outer insulator (1e-4 cm) gets u segments, the two 5e-3 cm
+    layers 10 u each, the core the remaining 42 u with steps growing geometrically from the core /
+    insulator interface towards the axis (first step = the insulator's).  Interfaces sit on nodes.
+    Returns (r, interface node indices)."""
+    assert (nr - 1) % 63 == 0 and nr >= 64, "nr - 1 must be a multiple of 63"
+    u = (nr - 1) // 63
+    r0, r1, r2, r3 = PAPER_RADII_CM
+    n_core, n1, n2, n3 = 42 * u, 10 * u, 10 * u, u
+    h1 = (r1 - r0) / n1
+    # core: steps h1 * q^k, k = 0 .. n_core-1 from the interface inwards, summing to r0
+    lo, hi = 1.0, 2.0
+    for _ in range(200):
+        q = (lo + hi) / 2
+        tot = h1 * n_core if abs(q - 1) < 1e-15 else h1 * (q ** n_core - 1) / (q - 1)
+        lo, hi = (q, hi) if tot < r0 else (lo, q)
+    hk = h1 * q ** np.arange(n_core)
+    hk *= r0 / hk.sum()
+    core = r0 - np.concatenate([[0.0], np.cumsum(hk)])          # r0 ... 0
+    core = core[::-1].copy()
+    core[0] = 0.0
+    seg1 = r0 + (r1 - r0) * np.arange(1, n1 + 1) / n1
+    seg2 = r1 + (r2 - r1) * np.arange(1, n2 + 1) / n2
+    seg3 = r2 + (r3 - r2) * np.arange(1, n3 + 1) / n3
+    r = np.concatenate([core, seg1, seg2, seg3])
+    assert r.size == nr and np.all(np.diff(r) > 0)
+    return r, [n_core, n_core + n1, n_core + n1 + n2]
+
+
+def paper_device(M=201, nr=631, tau=1e-5, printed_graphite=False):
+    """The workload of the paper's section 5: radii 0.12 / 0.125 / 0.13 / 0.1301 cm,
+    z_max = 5 cm, POLY laws of Tables 2-3, source chi(T) I_0^2 / S_2^2 in the conducting layer with
+    I_0 = 363 mA, zero flux everywhere except T = 4.2 K at z_max (6), T_0 = 4.2 K, tau = 1e-5 s,
+    t_prd = 25 ms, t_src = 1 ms, 100 transient sub-steps.  M = axial nodes (201 ... 1201, Table 4).
+    Missing from the paper and filled in here: the radial node distribution (paper_radial_nodes) and
+    the graphite c_V misprint (PAPER_GRAPHITE_A3_SUBSTITUTE).  CGS-like units: cm, g, s, W, J, K."""
+    r, ifaces = paper_radial_nodes(nr)
+    s = _base(nr, M, 1, 1, paper_layers(printed_graphite), seg_layers(nr, ifaces))
+    s["r"] = r
+    s["z"] = uniform_nodes(PAPER_ZMAX_CM, M)
+    s["r_in"], s["r_out"], s["z_lo"], s["z_hi"] = NEUMANN0, NEUMANN0, NEUMANN0, dirichlet(PAPER_T0)
+    s["T0"] = PAPER_T0
+    S2 = math.pi * (PAPER_RADII_CM[2] ** 2 - PAPER_RADII_CM[1] ** 2)
+    s["Q0"] = np.array([PAPER_CHI0 * PAPER_I0_A ** 2 / S2 ** 2])     # W/cm^3 times T^-1/2
+    s["dt"] = float(tau)
+    s["steps_per_period"] = int(round(25e-3 / tau))
+    s["steps_on"] = int(round(1e-3 / tau))
+    s["transient_substeps"], s["transient_k"] = 100, 7.0
+    s["T_lo"], s["T_hi"] = 4.2, 60.0
+    s["probes"] = [(nr - 1, 0), (nr - 1, M // 2), (0, 0)]           # Fig. 7 probe, mid surface, axis
+    s["probe_every"] = 1
+    s["name"] = f"paper device {nr}x{M}"
+    return s

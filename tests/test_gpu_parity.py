@@ -190,9 +190,10 @@ TBAND_CASES = [
     (1024, 21, 2, False, BC_SETS[2], 4),       # two warps per line, Dirichlet r boundaries
     (2048, 19, 1, True, BC_SETS[3], 4),        # a CTA per line
     (4096, 12, 1, False, None, 4),             # cluster of 2 CTAs per line
+    (4096, 10, 2, True, BC_SETS[2], 8),        # a CTA of 8 warps per line (default for nr = 4096)
     (8192, 7, 1, False, BC_SETS[1], 4),        # cluster of 4, Neumann z_lo
     (8192, 6, 2, True, None, 8),               # cluster of 2 CTAs of 8 warps
-    (8192, 9, 1, False, BC_SETS[3], 16),       # one CTA of 16 warps per line, no cluster
+    (8192, 9, 1, False, BC_SETS[3], 16),       # one CTA of 16 warps per line, no cluster (default for nr = 8192)
 ]
 
 
