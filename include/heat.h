@@ -172,10 +172,17 @@ const char *heat_last_error(const heat_ctx *c);
 
 void heat_destroy(heat_ctx *c);
 
-/* Measured-peak helper for the roofline: runs a dependent-chain-free DFMA loop on every SM
- * and returns the achieved fp64 FMA rate in TFLOP/s (2 flops per FMA); iters per thread.
- * Not part of the method; allocates and frees its own small scratch buffer. */
-heat_status heat_fp64_peak(int64_t iters, void *cuda_stream, double *tflops);
+/* ---- bench accounting (HEAT_BENCH): not part of the method ------------------------------------
+ * heat_launch_count and heat_kernel_name above belong here as well: they exist so that bench.py
+ * can report `gpu_launches` and name the kernel its roofline line is about.
+ *
+ * Measured-peak helper for the ALU co-limit of the roofline: runs a dependent-chain-free DFMA loop on
+ * every SM and returns the achieved fp64 FMA rate in TFLOP/s (2 flops per FMA); iters per thread.
+ *   scratch, scratch_bytes : caller-owned device buffer, >= heat_fp64_peak_scratch_bytes() bytes
+ *                            (like every other call, the library allocates no device memory)
+ * Synchronises cuda_stream. */
+size_t heat_fp64_peak_scratch_bytes(void);
+heat_status heat_fp64_peak(int64_t iters, void *scratch, size_t scratch_bytes, void *cuda_stream, double *tflops);
 
 #ifdef __cplusplus
 }

@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "HEAT_OK", 1: "HEAT_EINVAL", 2: "HEAT_ENOMEM", 3: "HEAT_ECUDA
 EXPORTS = [
     "heat_workspace_bytes", "heat_stable_dt", "heat_create", "heat_step", "heat_get_field",
     "heat_set_field", "heat_probe", "heat_schedule", "heat_step_index", "heat_launch_count",
-    "heat_kernel_name", "heat_last_error", "heat_destroy", "heat_fp64_peak",
+    "heat_kernel_name", "heat_last_error", "heat_destroy", "heat_fp64_peak", "heat_fp64_peak_scratch_bytes",
 ]
 
 
@@ -104,7 +104,9 @@ def lib():
         L.heat_destroy.restype = None
         L.heat_destroy.argtypes = [vp]
         L.heat_fp64_peak.restype = C.c_int
-        L.heat_fp64_peak.argtypes = [i64, vp, C.POINTER(dbl)]
+        L.heat_fp64_peak.argtypes = [i64, vp, C.c_size_t, vp, C.POINTER(dbl)]
+        L.heat_fp64_peak_scratch_bytes.restype = C.c_size_t
+        L.heat_fp64_peak_scratch_bytes.argtypes = []
         _lib = L
     return _lib
 
@@ -138,7 +140,7 @@ def _dptr(a):
 class Desc:
     """A heat_desc plus the numpy arrays that keep its host pointers alive."""
 
-    def __init__(self, spec, T_init_device_ptr=None):
+    def __init__(self, spec, T_init_device_ptr=None, placeholder_dt=False):
         self.r = np.ascontiguousarray(spec["r"], dtype=np.float64)
         self.z = np.ascontiguousarray(spec["z"], dtype=np.float64)
         nr, nz = self.r.size, self.z.size
@@ -170,7 +172,8 @@ class Desc:
             d.T_init, d.T_init_is_device = C.c_void_p(self.T_init.ctypes.data), 0
         else:
             d.T_init, d.T_init_is_device = None, 0
-        d.dt = float(spec.get("dt") or 1.0)
+        # heat_stable_dt / heat_workspace_bytes are asked before tau is known: only they may pass a placeholder
+        d.dt = float(spec.get("dt") or (1.0 if placeholder_dt else 0.0))
         d.Q0 = _dptr(self.Q0)
         d.steps_per_period = int(spec.get("steps_per_period", 0))
         d.steps_on = int(spec.get("steps_on", 0))
@@ -189,7 +192,7 @@ class Desc:
 
 def heat_stable_dt(spec, T_lo=None, T_hi=None) -> float:
     """Right-hand side of (21) P:L194-196 (host-only call of the C ABI)."""
-    m = Desc(spec)
+    m = Desc(spec, placeholder_dt=True)
     out = C.c_double()
     T_lo = float(spec["T_lo"] if T_lo is None else T_lo)
     T_hi = float(spec["T_hi"] if T_hi is None else T_hi)
@@ -200,13 +203,16 @@ def heat_stable_dt(spec, T_lo=None, T_hi=None) -> float:
 
 
 def heat_workspace_bytes(spec) -> int:
-    return int(lib().heat_workspace_bytes(C.byref(Desc(spec).desc)))
+    return int(lib().heat_workspace_bytes(C.byref(Desc(spec, placeholder_dt=True).desc)))
 
 
 def heat_fp64_peak(iters=1 << 16) -> float:
     import torch
     out = C.c_double()
-    st = lib().heat_fp64_peak(int(iters), C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out))
+    nbytes = int(lib().heat_fp64_peak_scratch_bytes())
+    scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    st = lib().heat_fp64_peak(int(iters), C.c_void_p(scratch.data_ptr()), nbytes,
+                              C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out))
     if st != HEAT_OK:
         raise HeatError(st, lib().heat_last_error(None).decode())
     return out.value
@@ -232,7 +238,10 @@ class HeatSim:
         cells = m.batch * m.nz * m.nr
         ws = int(self._L.heat_workspace_bytes(C.byref(m.desc)))
         if ws == 0:
-            raise HeatError(HEAT_EINVAL, self._L.heat_last_error(None).decode() or "descriptor rejected")
+            # heat_create validates the descriptor before it looks at the buffers: ask it for the real status
+            h0 = C.c_void_p()
+            st0 = self._L.heat_create(C.byref(m.desc), None, None, None, 0, None, 0, C.c_void_p(self.stream.cuda_stream), C.byref(h0))
+            raise HeatError(st0 if st0 != HEAT_OK else HEAT_EINVAL, self._L.heat_last_error(None).decode() or "descriptor rejected")
         dev = torch.device("cuda", torch.cuda.current_device())
         with torch.cuda.stream(self.stream):
             self.field_a = torch.empty(cells, dtype=torch.float64, device=dev)

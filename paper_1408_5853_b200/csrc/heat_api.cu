@@ -228,9 +228,12 @@ const BandVariant *plan_band(const heat_desc *d, std::vector<PLayer> *players, s
     if (d->face_mode != 0 || d->nz < 4) return nullptr;
     const int nr = d->nr, N = nr - 1;
     if (d->r[0] != 0.0) return nullptr;
+    // uniform means r_i == R i / N to a few ulp of R: the kernel generates (i +- 1/2) / h^2 on the fly,
+    // the oracle uses the r it is given, and the difference must stay far below the parity budget
+    // (a grid accumulated as r_i = r_{i-1} + h drifts by ~N ulp and takes the general kernels)
     const long double h = (long double)d->r[N] / (long double)N;
     for (int i = 1; i <= N; ++i)
-        if (fabsl((long double)d->r[i] - h * i) > 1e-13L * (long double)d->r[N]) return nullptr;
+        if (fabsl((long double)d->r[i] - h * i) > 4.0L * 2.220446049250313e-16L * (long double)d->r[N]) return nullptr;
     int degk = 0;
     std::vector<PLayer> pl((size_t)d->nlayers);
     for (int m = 0; m < d->nlayers; ++m) {
@@ -283,9 +286,12 @@ const WBandVariant *plan_wband(const heat_desc *d, std::vector<PLayer> *players,
     if (d->face_mode != 0 || d->nz < 4) return nullptr;
     const int nr = d->nr, N = nr - 1;
     if (d->r[0] != 0.0) return nullptr;
+    // uniform means r_i == R i / N to a few ulp of R: the kernel generates (i +- 1/2) / h^2 on the fly,
+    // the oracle uses the r it is given, and the difference must stay far below the parity budget
+    // (a grid accumulated as r_i = r_{i-1} + h drifts by ~N ulp and takes the general kernels)
     const long double h = (long double)d->r[N] / (long double)N;
     for (int i = 1; i <= N; ++i)
-        if (fabsl((long double)d->r[i] - h * i) > 1e-13L * (long double)d->r[N]) return nullptr;
+        if (fabsl((long double)d->r[i] - h * i) > 4.0L * 2.220446049250313e-16L * (long double)d->r[N]) return nullptr;
     int degk = 0;
     std::vector<PLayer> pl((size_t)d->nlayers);
     for (int m = 0; m < d->nlayers; ++m) {
@@ -759,7 +765,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (const char *eo = getenv("HEAT_BLOCKS_PER_SM")) occ_cap_env = std::max(1, atoi(eo));
     if (tv) {
         c->smem = tv->smem_fixed + sizeof(DLayer) * (size_t)d->nlayers;
-        e = cudaFuncSetAttribute((const void *)tv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+        // the attribute belongs to the kernel function, not to this context (several contexts with
+        // different layer counts may be alive): reserve the worst case
+        e = cudaFuncSetAttribute((const void *)tv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(tv->smem_fixed + sizeof(DLayer) * (size_t)HEAT_MAX_LAYERS));
         if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", tv->name, c->smem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
         const int lpb = 128 / tv->G;
         const int spm = (nz - 2 + lpb - 1) / lpb; // slabs per batch member
@@ -812,7 +821,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         c->tp.total_slabs = (int)total_slabs;
     } else {
         c->smem = v->smem_fixed + sizeof(DLayer) * (size_t)d->nlayers;
-        e = cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+        e = cudaFuncSetAttribute((const void *)v->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(v->smem_fixed + sizeof(DLayer) * (size_t)HEAT_MAX_LAYERS));
         if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", v->name, c->smem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
         int occ = 0;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)v->fn, v->tpb, c->smem);
@@ -826,7 +836,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     // ---- band kernel: launch shape, band partition, tensor maps
     if (bv) {
         const size_t bsmem = bv->smem_fixed + sizeof(PLayer) * (size_t)d->nlayers;
-        e = cudaFuncSetAttribute((const void *)bv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsmem);
+        e = cudaFuncSetAttribute((const void *)bv->fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(bv->smem_fixed + sizeof(PLayer) * (size_t)HEAT_MAX_LAYERS));
         if (e != cudaSuccess) { set_err(nullptr, "%s: cannot reserve %zu bytes of shared memory: %s", bv->name, bsmem, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
         int max_clusters = 0;
         {
@@ -1170,16 +1181,18 @@ const char *heat_kernel_name(const heat_ctx *c) { return c ? (c->tbvar ? c->tbva
 const char *heat_last_error(const heat_ctx *c) { return c ? c->err.c_str() : g_last_error.c_str(); }
 void heat_destroy(heat_ctx *c) { delete c; }
 
-heat_status heat_fp64_peak(int64_t iters, void *cuda_stream, double *tflops)
+size_t heat_fp64_peak_scratch_bytes(void) { return sizeof(double) * 1024u * 2u * 1024u; }
+
+heat_status heat_fp64_peak(int64_t iters, void *scratch, size_t scratch_bytes, void *cuda_stream, double *tflops)
 {
-    if (!tflops || iters < 1) return HEAT_EINVAL;
+    if (!tflops || iters < 1 || !scratch) return HEAT_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
     CUDA_TRY(nullptr, cudaGetDevice(&dev));
     CUDA_TRY(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int tpb = 1024, blocks = sms * 2;
-    double *out = nullptr;
-    CUDA_TRY(nullptr, cudaMalloc(&out, sizeof(double) * (size_t)tpb * blocks));
+    if (scratch_bytes < sizeof(double) * (size_t)tpb * blocks) { set_err(nullptr, "heat_fp64_peak: scratch too small"); return HEAT_ENOMEM; }
+    double *out = (double *)scratch;
     cudaEvent_t e0, e1;
     CUDA_TRY(nullptr, cudaEventCreate(&e0));
     CUDA_TRY(nullptr, cudaEventCreate(&e1));
@@ -1193,7 +1206,6 @@ heat_status heat_fp64_peak(int64_t iters, void *cuda_stream, double *tflops)
     *tflops = 2.0 * 8.0 * (double)iters * tpb * blocks / (ms * 1e-3) / 1e12;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(out);
     return HEAT_OK;
 }
 

@@ -466,3 +466,40 @@ def test_config4_windows(bd):
     pg, dropped = sim.probes()
     assert pg.shape == (100, 1, 1) and dropped == 0
     assert abs(pg[-1, 0, 0] - orc.field(0)[s["probes"][0][1], s["probes"][0][0]]) <= TOL
+
+
+# ----------------------------------------------------------------------------- the paper's own device (f1)
+
+def test_paper_device_windows(bd):
+    """SURVEY 8(f) f1, the workload of the paper's section 5 on its 631 x 201 grid (non-uniform r,
+    POLY laws of Tables 2-3, chi(T) ~ T^-1/2 source, Neumann z = 0 / Dirichlet 4.2 K at z_max):
+    from the initial condition through the 100 transient sub-steps, across switch-off (snapshot
+    seeded) and across the next switch-on."""
+    s = I.paper_device(201)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s, variant="omp")
+    per = s["steps_per_period"] - 1 + s["transient_substeps"]
+    off = s["transient_substeps"] + s["steps_on"] - 1
+    sim.step(150); orc.step(150)                      # W1: sub-steps + the first tau steps
+    compare(sim, orc)
+    sim.step(off - 150 - 20)                          # GPU alone up to 20 steps before switch-off
+    orc.set_field(0, sim.field(0), sim.step_index)
+    sim.step(60); orc.step(60)                        # W2: across switch-off
+    compare(sim, orc)
+    sim.step(per - sim.step_index - 30)               # ... up to 30 steps before the next switch-on
+    orc.set_field(0, sim.field(0), sim.step_index)
+    sim.step(160); orc.step(160)                      # W3: across switch-on and its sub-steps
+    compare(sim, orc)
+    pg, _ = sim.probes()
+    assert np.all(np.isfinite(pg)) and pg[:, 0, 0].max() > 8.0   # the surface probe of Fig. 7 warms up
+    sim.close()
+
+
+def test_paper_device_downscaled_forty_periods(bd):
+    """The same physics on 64 x 21 nodes over 40 source periods (104 000 solver steps): drift."""
+    s = I.paper_device(21, nr=64)
+    sim, orc = bd.HeatSim(s, probe_records=8), oracle_cls()(s)
+    n = 40 * (s["steps_per_period"] - 1 + s["transient_substeps"])
+    sim.step(n); orc.step(n)
+    err = compare(sim, orc)
+    assert sim.field(0).max() > 6.0
+    sim.close()

@@ -32,3 +32,60 @@ def test_band_spec_is_seeded():
     a, b, c = I.band_spec(5, nr=512, nz=12), I.band_spec(5, nr=512, nz=12), I.band_spec(6, nr=512, nz=12)
     assert np.array_equal(a["T_init"], b["T_init"]) and np.array_equal(a["seg_layer"], b["seg_layer"])
     assert not np.array_equal(a["T_init"], c["T_init"])
+
+
+def _golden():
+    import os
+    out = {"cv": {}, "lam": {}, "rho": {}}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_tables_2_3.txt")):
+        f = line.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] in ("cv", "lam"):
+            out[f[0]][int(f[1])] = tuple(float(x) for x in f[2:])
+        elif f[0] == "rho":
+            out["rho"][int(f[1])] = float(f[2])
+    return out
+
+
+def test_paper_device_uses_the_papers_printed_numbers():
+    """inputs.paper_device carries Tables 2-3 and the densities exactly as printed
+    (tests/golden/paper_tables_2_3.txt), except for the ONE stated substitution in the
+    graphite c_V row; geometry, source and schedule are P:L241, L274-278."""
+    g = _golden()
+    for m in range(4):
+        assert I.PAPER_CV_DESC[m] == g["cv"][m] and I.PAPER_LAM_DESC[m] == g["lam"][m]
+        assert I.PAPER_RHO[m] == g["rho"][m]
+    s = I.paper_device(201)
+    assert s["nr"] == 631 and s["nz"] == 201 and s["dt"] == 1e-5
+    assert s["steps_per_period"] == 2500 and s["steps_on"] == 100 and s["transient_substeps"] == 100
+    r = s["r"]
+    seg = s["seg_layer"][0]
+    nodes = np.flatnonzero(np.diff(seg.astype(int))) + 1
+    assert np.allclose(r[nodes], I.PAPER_RADII_CM[:3], rtol=1e-13) and r[-1] == pytest.approx(0.1301, rel=1e-13) and r[0] == 0.0
+    # every thin layer is resolved by >= 10 radial steps (P:L290)
+    assert nodes[1] - nodes[0] >= 10 and nodes[2] - nodes[1] >= 10 and 630 - nodes[2] >= 10
+    assert s["Q0"][0] == pytest.approx(1.8 * 0.363 ** 2 / (np.pi * (0.13 ** 2 - 0.125 ** 2)) ** 2, rel=1e-14)
+    lay = s["layers"]
+    assert lay[2]["is_heater"] and lay[2]["src_shape"]["c"][1] == -0.5
+    assert lay[2]["cp"]["c"][::-1][0] == I.PAPER_GRAPHITE_A3_SUBSTITUTE          # the substitution, and only there
+    assert tuple(lay[1]["cp"]["c"][::-1]) == g["cv"][1] and tuple(lay[3]["k"]["c"][::-1]) == g["lam"][3]
+
+
+def test_library_rejects_the_printed_graphite_row():
+    """Reading G11: the graphite c_V row as printed is negative above 22 K; the library's descriptor
+    validation (no device needed) refuses it and accepts the substituted row."""
+    from paper_1408_5853_b200 import binding
+    assert binding.heat_workspace_bytes(I.paper_device(201)) > 0
+    assert binding.heat_workspace_bytes(I.paper_device(201, printed_graphite=True)) == 0
+
+
+def test_paper_device_runs_on_the_oracle():
+    from oracle.heat_oracle import Oracle, stable_dt
+    s = I.paper_device(41, nr=64)
+    assert s["dt"] < stable_dt(s) * 26       # (21) at M = 41 is 25 x the M = 201 bound; tau = 1e-5 is far inside
+    o = Oracle(s)
+    o.step(260)
+    T = o.field()
+    assert np.all(np.isfinite(T)) and T.min() >= 4.2 - 1e-9 and T.max() > 6.0     # the heater warms up during the 1 ms pulse
+    assert np.all(T[-1] == 4.2)                                                   # Dirichlet terminal at z_max
