@@ -221,7 +221,7 @@ def heat_fp64_peak(iters=1 << 16) -> float:
 class HeatSim:
     """One simulation context on the current CUDA device: heat_create .. heat_destroy."""
 
-    def __init__(self, spec, probe_records=None, stream=None, T_init_device=None):
+    def __init__(self, spec, probe_records=None, stream=None, T_init_device=None, guard=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("HeatSim needs a CUDA device (B200, sm_100a); there is no CPU fallback")
@@ -244,14 +244,28 @@ class HeatSim:
             raise HeatError(st0 if st0 != HEAT_OK else HEAT_EINVAL, self._L.heat_last_error(None).decode() or "descriptor rejected")
         dev = torch.device("cuda", torch.cuda.current_device())
         with torch.cuda.stream(self.stream):
-            self.field_a = torch.empty(cells, dtype=torch.float64, device=dev)
-            self.field_b = torch.empty(cells, dtype=torch.float64, device=dev)
-            self.workspace = torch.empty(ws, dtype=torch.uint8, device=dev)
             rec = m.batch * m.nprobes
             if probe_records is None:
                 probe_records = 4096
             self.probe_cap = max(rec * int(probe_records), 1)
-            self.probe_buf = torch.zeros(self.probe_cap, dtype=torch.float64, device=dev)
+            # guard > 0 (tests): every buffer the library is handed sits between two bands of `guard`
+            # doubles holding a canary, so that a write outside a buffer is seen (guards_intact)
+            g = int(guard)
+            self._guards = []
+
+            def banded(n):
+                big = torch.full((n + 2 * g,), self.CANARY, dtype=torch.float64, device=dev)
+                if g:
+                    self._guards += [big[:g], big[g + n:]]
+                return big[g:g + n]
+
+            self.field_a = banded(cells)
+            self.field_b = banded(cells)
+            self._ws64 = banded((ws + 7) // 8 + 32)
+            ws_off = (-self._ws64.data_ptr()) % 256                # the workspace must be 256-byte aligned
+            self.workspace = self._ws64.view(torch.uint8)[ws_off:ws_off + ws]
+            self.probe_buf = banded(self.probe_cap)
+            self.probe_buf.zero_()
         h = C.c_void_p()
         st = self._L.heat_create(C.byref(m.desc), self.field_a.data_ptr(), self.field_b.data_ptr(),
                                  self.workspace.data_ptr(), ws, self.probe_buf.data_ptr(), self.probe_cap,
@@ -259,6 +273,12 @@ class HeatSim:
         if st != HEAT_OK:
             raise HeatError(st, self._L.heat_last_error(None).decode())
         self._h = h
+
+    CANARY = -7.0e77
+
+    def guards_intact(self) -> bool:
+        self.stream.synchronize()
+        return all(bool((b == self.CANARY).all().item()) for b in self._guards)
 
     # -- C ABI calls ------------------------------------------------------------------
     def _check(self, st):

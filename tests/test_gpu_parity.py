@@ -503,3 +503,112 @@ def test_paper_device_downscaled_forty_periods(bd):
     err = compare(sim, orc)
     assert sim.field(0).max() > 6.0
     sim.close()
+
+
+# ----------------------------------------------------------------------------- round-2 parity holes / ADVICE
+
+def test_thin_grid_drift_is_rounding_not_the_kernel(bd):
+    """test_every_kernel_variant keeps eta = 10 h.  Here the grid is the thin
+    one that test avoids (L/R = 10 with nz << nr, eta = 550 h): the line systems are ill-conditioned
+    and fp64 rounding alone moves the result.  Measured statement instead of a narrowed input: the GPU
+    differs from the long-double oracle by no more than a small multiple of what the fp64 oracle
+    itself differs from it."""
+    s = with_dt(bd, I.config(2, nr=1021, nz=12))
+    sim, o64, o80 = bd.HeatSim(s), oracle_cls()(s), oracle_cls()(s, variant="long")
+    assert sim.kernel_name.startswith("line<")
+    sim.step(120); o64.step(120); o80.step(120)
+    ref = o80.field(0)
+    floor = float(np.max(np.abs(o64.field(0) - ref)))
+    gpu = float(np.max(np.abs(sim.field(0) - ref)))
+    print(f"thin grid: |fp64 oracle - long double| = {floor:.3e} K, |GPU - long double| = {gpu:.3e} K")
+    assert gpu <= 3.0 * floor + 1e-12
+    sim.close()
+
+
+@pytest.mark.parametrize("nr,r0", [(128, 0.0), (128, 3e-4), (256, 0.0), (256, 2e-4)])
+def test_tma_kernel_on_nonuniform_r(bd, nr, r0, monkeypatch):
+    """the TMA kernel's table-driven rows on a NON-uniform r grid and on a grid
+    that starts at r_0 > 0 (pick_tma_variant routes nr = 128 .. 8192 there when the band kernels decline)."""
+    monkeypatch.setenv("HEAT_KERNEL", "tma")
+    s = I.random_spec(nr, nr=nr, nz=14, nlayers=3, batch=2, r0=r0, bcs=BC_SETS[(nr // 128 + (r0 > 0)) % 4])
+    s = with_dt(bd, s, 0.8)
+    sim, orc = bd.HeatSim(s), oracle_cls()(s)
+    assert sim.kernel_name.startswith("tma<"), sim.kernel_name
+    for n in (1, 7, 12):
+        sim.step(n); orc.step(n)
+        compare(sim, orc)
+    pg, _ = sim.probes()
+    assert np.max(np.abs(pg - orc.probes())) <= TOL
+    sim.close()
+
+
+def test_almost_uniform_grid_takes_the_general_kernel(bd):
+    """the kernels that generate (i +- 1/2) / h^2 on the fly accept a grid only if it is
+    R i / N to a few ulp of R (the oracle uses the r it is given).  A grid that is off by 1e-12 R in
+    places -- thousands of ulp, yet far below anything a tolerance on h would notice -- must go to the
+    general kernel and match the oracle there; a grid accumulated as r_i = r_{i-1} + h stays within a
+    few ulp and may take the fast kernel, where it must match as well."""
+    base = I.config(2, nr=512, nz=16)
+    R = base["r"][-1]
+    bent = dict(base, r=base["r"].copy())
+    bent["r"][100:300] += 1e-12 * R
+    acc = dict(base, r=np.concatenate([[0.0], np.cumsum(np.full(511, R / 511))]))
+    for spec, must_be_general in ((bent, True), (acc, False), (base, False)):
+        s = with_dt(bd, spec)
+        sim, orc = bd.HeatSim(s), oracle_cls()(s)
+        fast = sim.kernel_name.startswith(("tband<", "wband<", "band<"))
+        assert not (fast and must_be_general), sim.kernel_name
+        if spec is base:
+            assert sim.kernel_name.startswith("tband<"), sim.kernel_name
+        sim.step(150); orc.step(150)
+        compare(sim, orc)
+        sim.close()
+
+
+def test_two_live_contexts_with_different_layer_counts(bd):
+    """the dynamic shared-memory attribute belongs to the kernel function; a context
+    with fewer layers created after one with more must not break the launches of the first."""
+    for nr in (512, 96):                                      # tband kernel / line kernel
+        a = bd.HeatSim(with_dt(bd, I.config(2, nr=nr, nz=24)))                 # 4 layers
+        two = I.config(0, nr=nr, nz=24)                                        # 3 layers
+        b = bd.HeatSim(with_dt(bd, two))
+        a.step(20); b.step(20); a.step(20)
+        oa, ob = oracle_cls()(with_dt(bd, I.config(2, nr=nr, nz=24))), oracle_cls()(with_dt(bd, two))
+        oa.step(40); ob.step(20)
+        compare(a, oa); compare(b, ob)
+        a.close(); b.close()
+
+
+def test_missing_dt_is_rejected(bd):
+    """a spec without tau must fail in heat_create, not run with a placeholder."""
+    s = I.config(1, nr=64, nz=32)
+    assert s["dt"] is None
+    with pytest.raises(bd.HeatError):
+        bd.HeatSim(s)
+
+
+GUARD_CASES = [({}, 1024, 8, 2), ({"HEAT_TBAND_NW": "16"}, 8192, 6, 1), ({"HEAT_TBAND_NW": "4"}, 8192, 6, 1),
+               ({"HEAT_TBAND_NW": "8"}, 4096, 7, 2), ({"HEAT_KERNEL": "wband"}, 4096, 6, 1), ({"HEAT_KERNEL": "band"}, 4096, 6, 1),
+               ({"HEAT_KERNEL": "band"}, 512, 8, 2), ({"HEAT_KERNEL": "tma"}, 256, 8, 2), ({"HEAT_KERNEL": "line"}, 96, 8, 2)]
+
+
+@pytest.mark.parametrize("case", GUARD_CASES, ids=lambda c: "-".join(f"{k[5:]}{v}" for k, v in c[0].items()) + f"nr{c[1]}")
+def test_no_write_outside_the_callers_buffers(bd, case, monkeypatch):
+    """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so the out-of-bounds
+    check is our own: both field levels, the workspace and the probe ring sit between canary bands of
+    4096 doubles; after a run with TMA stores on the first / last lines, Neumann z copies, probes on
+    boundary nodes and a ragged band partition every band still holds its canary, for every kernel family."""
+    env, nr, nz, batch = case
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    s = I.band_spec(nr + nz, nr=nr, nz=nz, batch=batch, chunk=16, bcs=BC_SETS[1] if nr % 1024 else BC_SETS[3])
+    s = with_dt(bd, s, 0.8)
+    sim = bd.HeatSim(s, guard=4096, probe_records=3)      # the probe ring overflows on purpose (records are dropped, not written past)
+    sim.step(11)
+    assert sim.guards_intact(), sim.kernel_name
+    orc = oracle_cls()(s, variant="omp" if nr * nz > 30000 else "double")
+    orc.step(11)
+    compare(sim, orc)
+    pg, dropped = sim.probes()
+    assert pg.shape[0] == 3 and dropped == 11 // s["probe_every"] - 3 and sim.guards_intact()
+    sim.close()
