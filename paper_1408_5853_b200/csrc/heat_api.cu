@@ -39,7 +39,7 @@ void set_err(std::string *dst, const char *fmt, ...)
 typedef void (*kernel_fn)(const KParams);
 struct Variant {
     int M, G, tpb, lpb;
-    kernel_fn fn;
+    kernel_fn fn, fn_persist;
     const char *name;
     size_t smem_fixed; // bytes without the layer table
 };
@@ -47,6 +47,7 @@ struct Variant {
 #define HEAT_VARIANT(M_, G_)                                                                      \
     {                                                                                             \
         M_, G_, LineCfg<M_, G_>::TPB, LineCfg<M_, G_>::LPB, heat_line_kernel<M_, G_>,             \
+            heat_line_persist_kernel<M_, G_>,                                                     \
             "line<M=" #M_ ",G=" #G_ ">", LineCfg<M_, G_>::smem_bytes(0)                           \
     }
 const Variant k_variants[] = {
@@ -358,7 +359,7 @@ constexpr int k_range_samples = 1025;
 // ---------------------------------------------------------------- workspace layout
 struct Layout {
     int nrp;
-    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, off_wdesc, total;
+    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, off_wdesc, off_ampsub, total;
 };
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -380,6 +381,7 @@ Layout make_layout(const heat_desc *d, const Variant *v, const TmaVariant *tv)
     L.off_bdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 8 + 1), 256);
     L.off_players = o; o = align_up(o + sizeof(PLayer) * (size_t)HEAT_MAX_LAYERS, 256);
     L.off_wdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 16 + 1), 256);
+    L.off_ampsub = o; o = align_up(o + sizeof(double) * (size_t)(d->transient_substeps + 1), 256);
     L.total = o;
     return L;
 }
@@ -461,6 +463,7 @@ struct heat_ctx {
     WParams wp;
     CUtensorMap wtm[2]; // [0] = field_a, [1] = field_b; box {16, 32}
     int pdl;                 // band kernel: launch with programmatic stream serialization
+    int persist;             // line kernel: heat_step(n >= 2) is one cooperative multi-step launch
     CUtensorMap btm_ld[2], btm_st[2];
     BParams bp;
     CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
@@ -589,12 +592,12 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     c->var = v; c->tvar = tv; c->bvar = bv; c->wvar = wv; c->tbvar = tbv; c->lay = L; c->ws = (char *)workspace;
     // measured: 10.4 -> 8.7 us per step on 512 x 512, 36.9 -> 34.7 on 2048 x 2048; with clusters (nr >= 4096)
     // the piecemeal placement of the next step's clusters costs 11 %, so it stays off there
-    c->pdl = ((bv && bv->CL == 1) || (wv && !tbv && wv->CL == 1)) ? 1 : 0;
+    c->pdl = ((bv && bv->CL == 1) || (wv && !tbv && wv->CL == 1) || (tbv && tbv->CL == 1)) ? 1 : 0;
     if (const char *ep = getenv("HEAT_PDL")) c->pdl = atoi(ep) != 0;
     c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
     c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
-    c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0;
+    c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0; c->persist = 0;
 
     // ---- per-node row tables (host), SURVEY 8(a) a4
     const int nr = d->nr, nz = d->nz, N = nr - 1, nrp = L.nrp;
@@ -725,6 +728,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     UP(L.off_q0, q0, double);
     UP(L.off_probes, pr, ProbeSrc);
     UP(L.off_cdesc, cdesc, uint32_t);
+    if (!c->amp_sub.empty()) UP(L.off_ampsub, c->amp_sub, double);
     if (bv) {
         UP(L.off_bdesc, bdesc, uint32_t);
         UP(L.off_players, players, PLayer);
@@ -830,6 +834,16 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         const long long want = (total_lines + v->lpb - 1) / v->lpb;
         const int occ_cap = occ_cap_env > 0 ? std::min(occ, occ_cap_env) : occ;
         c->grid = (int)std::min<long long>(want, (long long)prop.multiProcessorCount * occ_cap);
+        // persistent multi-step launches: every CTA of the grid is resident (by the line above), so a
+        // cooperative launch with a grid barrier between the steps is legal
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        e = cudaFuncSetAttribute((const void *)v->fn_persist, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(v->smem_fixed + sizeof(DLayer) * (size_t)HEAT_MAX_LAYERS));
+        int occp = 0;
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, (const void *)v->fn_persist, v->tpb, c->smem);
+        c->persist = (coop && e == cudaSuccess && (long long)c->grid <= (long long)prop.multiProcessorCount * occp) ? 1 : 0;
+        if (const char *ep = getenv("HEAT_PERSIST")) c->persist = c->persist && atoi(ep) != 0;
     }
 
 
@@ -1033,6 +1047,11 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     k.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
     k.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
     k.total_lines = (int)total_lines;
+    k.probe_every = c->probe_every;
+    k.probe_base = c->probe_buf; k.probe_cap = c->probe_cap;
+    k.sched.P = c->P; k.sched.S = c->S; k.sched.nsub = c->nsub;
+    k.sched.inv_dt = 1.0 / c->dt; k.sched.inv_dt_sub = c->nsub > 0 ? 1.0 / (c->dt / (double)c->nsub) : 0.0;
+    k.sched.amp_sub = (const double *)(c->ws + L.off_ampsub);
 
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { set_err(nullptr, "stream sync failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
@@ -1045,6 +1064,30 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
     if (!c || n < 0) return HEAT_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t rec = (size_t)c->batch * (size_t)c->nprobes;
+    if (c->persist && !c->bvar && !c->tvar && !c->wvar && n >= 2) {
+        // one cooperative launch per chunk: schedule, level swap and probe slots run on the device
+        int64_t left = n;
+        while (left > 0) {
+            const int64_t chunk = std::min<int64_t>(left, 1 << 20);
+            KParams &k = c->kp;
+            k.Told = c->cur; k.Tnew = c->nxt;
+            k.nsteps = (int)chunk; k.step0 = c->step; k.rec0 = c->rec_enqueued;
+            void *args[] = {(void *)&k};
+            CUDA_TRY(&c->err, cudaLaunchCooperativeKernel((const void *)c->var->fn_persist, dim3((unsigned)c->grid), dim3((unsigned)c->var->tpb),
+                                                          args, c->smem, st));
+            c->launches += 1;
+            if (c->nprobes > 0) { // the host's mirror of the device's record arithmetic
+                const int64_t cnt = (c->step + chunk) / c->probe_every - c->step / c->probe_every;
+                const int64_t room = (int64_t)(c->probe_cap / rec) - c->rec_enqueued;
+                const int64_t fits = std::max<int64_t>(0, std::min(cnt, room));
+                c->rec_enqueued += fits; c->rec_dropped += cnt - fits;
+            }
+            if (chunk & 1) std::swap(c->cur, c->nxt);
+            c->step += chunk; left -= chunk;
+        }
+        CUDA_TRY(&c->err, cudaGetLastError());
+        return HEAT_OK;
+    }
     for (int64_t s = 0; s < n; ++s) {
         double tau, amp;
         heat_schedule(c, c->step, &tau, &amp);

@@ -116,6 +116,15 @@ struct ProbeSrc {
     int is_static;
 };
 
+// the step schedule on the device (persistent multi-step kernels): integer state -> (1/tau_k, amp_k)
+struct DSched {
+    long long P, S;      // steps per period / steps with the source on, in units of tau; 0 = no source
+    int nsub;            // transient sub-steps replacing the first tau of a period; 0 = Heaviside
+    int pad_;
+    double inv_dt, inv_dt_sub;
+    const double *amp_sub; // [nsub]: 1 - exp(-q / k), (22) P:L212 (reading G8)
+};
+
 struct KParams {
     const double *Told; // current level  [batch][nz][nr]
     double *Tnew;       // next level
@@ -135,6 +144,12 @@ struct KParams {
     int face_mode;
     int z_lo_neumann, z_hi_neumann;
     int total_lines;    // batch * (nz-2)
+    // persistent multi-step launch (heat_line_persist_kernel)
+    int nsteps, probe_every;
+    long long step0, rec0;
+    size_t probe_cap;
+    double *probe_base;
+    DSched sched;
 };
 
 } // namespace heat

@@ -16,6 +16,7 @@
 // The sweep coefficients never leave the SM (shared memory), so HBM sees 8 B read + 8 B
 // written per cell-update.
 #pragma once
+#include <cooperative_groups.h>
 #include "heat_device.cuh"
 
 namespace heat {
@@ -81,16 +82,18 @@ struct LineCfg {
     }
 };
 
-template <int M, int G>
-__global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __grid_constant__ KParams p)
+// field loads: read-only path for a one-step launch; for the persistent multi-step kernel the level
+// read in step k was written in step k-1 of the same launch, so it must come from L2 (ld.global.cg)
+template <bool COH, typename T>
+__device__ __forceinline__ T ldT(const T *ptr) { return COH ? __ldcg(ptr) : __ldg(ptr); }
+
+// One solver step of the lines this CTA owns (grid-stride over groups of LPB lines).
+template <int M, int G, bool COH>
+__device__ __forceinline__ void line_step(const KParams &p, const double *Told, double *Tnew, double inv_tau_k, double amp_k,
+                                          double *probe_out, double *st, double *xch, const DLayer *lay)
 {
     using Cfg = LineCfg<M, G>;
     constexpr int TPB = Cfg::TPB;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double *st = reinterpret_cast<double *>(smem_raw); // [3][M][TPB]
-    double *xch = st + 3 * M * TPB;                    // [10][NW]
-    DLayer *lay = reinterpret_cast<DLayer *>(xch + 10 * Cfg::NW);
-
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
@@ -99,11 +102,6 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
     const int i0 = t * M;      // first node of this thread
     const int wig = t >> 5;    // warp within the group
     const int gw0 = (grp * G) >> 5; // first warp of the group (MULTI only)
-
-    for (int q = tid; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
-        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
-    __syncthreads();
-
     const int nr = p.nr, nz = p.nz;
     const bool vec_ok = ((nr & 1) == 0);
     const int interior = nz - 2;
@@ -115,7 +113,7 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
         const int b = Lidx / interior;
         const int j = 1 + (Lidx - b * interior);
         const size_t line = ((size_t)b * nz + j) * (size_t)nr;
-        const double *Tl = p.Told + line;
+        const double *Tl = Told + line;
         const double *Tm = Tl - nr;
         const double *Tp = Tl + nr;
         const double *ga = p.ga + (size_t)b * p.nrp + i0;
@@ -128,19 +126,19 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
 #pragma unroll
             for (int k = 0; k < M; k += 2) {
                 double2 v = make_double2(1.0, 1.0);
-                if (i0 + k < nr) v = __ldg(reinterpret_cast<const double2 *>(Tl + i0 + k));
+                if (i0 + k < nr) v = ldT<COH>(reinterpret_cast<const double2 *>(Tl + i0 + k));
                 Tc[k + 1] = v.x; Tc[k + 2] = v.y;
             }
         } else {
 #pragma unroll
-            for (int k = 0; k < M; ++k) Tc[k + 1] = (i0 + k < nr) ? __ldg(Tl + i0 + k) : 1.0;
+            for (int k = 0; k < M; ++k) Tc[k + 1] = (i0 + k < nr) ? ldT<COH>(Tl + i0 + k) : 1.0;
         }
-        Tc[0] = (i0 > 0 && i0 - 1 < nr) ? __ldg(Tl + i0 - 1) : 1.0;
-        Tc[M + 1] = (i0 + M < nr) ? __ldg(Tl + i0 + M) : 1.0;
+        Tc[0] = (i0 > 0 && i0 - 1 < nr) ? ldT<COH>(Tl + i0 - 1) : 1.0;
+        Tc[M + 1] = (i0 + M < nr) ? ldT<COH>(Tl + i0 + M) : 1.0;
 
         const double ezm = __ldg(p.ezm + j), ezp = __ldg(p.ezp + j);
-        const double qa = __ldg(p.Q0 + b) * p.amp; // Q0 nu(t_k) p^2(t_k), (2)-(4),(22)
-        const double inv_tau = p.inv_tau;
+        const double qa = __ldg(p.Q0 + b) * amp_k; // Q0 nu(t_k) p^2(t_k), (2)-(4),(22)
+        const double inv_tau = inv_tau_k;
         const int fm = p.face_mode;
 
         // ---- level 1: assemble each row (13)/(15)/(18) and sweep it (12) at once
@@ -154,14 +152,14 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
                 if ((k & 1) == 0) {
                     double2 vm = make_double2(1.0, 1.0), vp = vm;
                     if (i0 + k < nr) {
-                        vm = __ldg(reinterpret_cast<const double2 *>(Tm + i0 + k));
-                        vp = __ldg(reinterpret_cast<const double2 *>(Tp + i0 + k));
+                        vm = ldT<COH>(reinterpret_cast<const double2 *>(Tm + i0 + k));
+                        vp = ldT<COH>(reinterpret_cast<const double2 *>(Tp + i0 + k));
                     }
                     Tdn2 = vm; Tup2 = vp;
                 }
             } else {
                 const bool ok = i0 + k < nr;
-                const double vm = ok ? __ldg(Tm + i0 + k) : 1.0, vp = ok ? __ldg(Tp + i0 + k) : 1.0;
+                const double vm = ok ? ldT<COH>(Tm + i0 + k) : 1.0, vp = ok ? ldT<COH>(Tp + i0 + k) : 1.0;
                 if ((k & 1) == 0) { Tdn2.x = vm; Tup2.x = vp; } else { Tdn2.y = vm; Tup2.y = vp; }
             }
             const double Tdn_k = (k & 1) ? Tdn2.y : Tdn2.x;
@@ -302,7 +300,7 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
 
         // ---- store T^ (and the Neumann z lines, which copy their neighbour; reading G16)
         if (live) {
-            double *out = p.Tnew + line;
+            double *out = Tnew + line;
             const bool lo = (j == 1) && p.z_lo_neumann;
             const bool hi = (j == nz - 2) && p.z_hi_neumann;
             if (vec_ok) {
@@ -326,23 +324,89 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
                 }
             }
             // ---- probes: T of the new level at (i_p, j_p)
-            if (p.probe_out != nullptr) {
+            if (probe_out != nullptr) {
                 for (int q = 0; q < p.nprobes; ++q) {
                     const ProbeSrc ps = p.probes[q];
                     if (ps.i < i0 || ps.i >= i0 + M) continue;
                     if (ps.is_static) {
-                        if (j == 1) p.probe_out[b * p.nprobes + q] = p.Told[((size_t)b * nz + ps.j_store) * nr + ps.i];
+                        if (j == 1) probe_out[b * p.nprobes + q] = Told[((size_t)b * nz + ps.j_store) * nr + ps.i];
                     } else if (ps.j_src == j) {
                         double v = 0.0;
 #pragma unroll
                         for (int k = 0; k < M; ++k)
                             if (i0 + k == ps.i) v = x[k];
-                        p.probe_out[b * p.nprobes + q] = v;
+                        probe_out[b * p.nprobes + q] = v;
                     }
                 }
             }
         }
         if (Cfg::MULTI) __syncthreads(); // xch is reused by the next line
+    }
+}
+
+template <int M, int G>
+__global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __grid_constant__ KParams p)
+{
+    using Cfg = LineCfg<M, G>;
+    constexpr int TPB = Cfg::TPB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *st = reinterpret_cast<double *>(smem_raw); // [3][M][TPB]
+    double *xch = st + 3 * M * TPB;                    // [10][NW]
+    DLayer *lay = reinterpret_cast<DLayer *>(xch + 10 * Cfg::NW);
+    for (int q = threadIdx.x; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
+        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
+    __syncthreads();
+    line_step<M, G, false>(p, p.Told, p.Tnew, p.inv_tau, p.amp, p.probe_out, st, xch, lay);
+}
+
+// (tau_k, amplitude_k) of solver step s from integer counters only: (4) P:L79 and (22) + procedure
+// P:L212-217 (readings G8, G9, G18); the device twin of heat_schedule in heat_api.cu.
+__device__ __forceinline__ void dev_schedule(const DSched &d, long long s, double &inv_tau, double &amp)
+{
+    if (d.P <= 0 || d.S <= 0) { inv_tau = d.inv_dt; amp = 0.0; return; }
+    if (d.nsub > 0) {
+        const long long len = (long long)d.nsub + d.P - 1; // solver steps per period
+        const long long q = s % len;
+        if (q < d.nsub) { inv_tau = d.inv_dt_sub; amp = d.amp_sub[q]; }
+        else { const long long g = q - d.nsub + 1; inv_tau = d.inv_dt; amp = (g < d.S) ? 1.0 : 0.0; }
+    } else {
+        inv_tau = d.inv_dt; amp = ((s % d.P) < d.S) ? 1.0 : 0.0;
+    }
+}
+
+// Persistent multi-step version for grids whose CTAs are all resident (cooperative launch): the
+// schedule runs on the device, the two levels swap roles every step, a grid-wide barrier separates the
+// steps.  One launch advances p.nsteps solver steps; this is what removes the launch latency that
+// dominates small grids (the paper's own Table 4 shows the same flat per-step cost).
+template <int M, int G>
+__global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_persist_kernel(const __grid_constant__ KParams p)
+{
+    using Cfg = LineCfg<M, G>;
+    constexpr int TPB = Cfg::TPB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *st = reinterpret_cast<double *>(smem_raw);
+    double *xch = st + 3 * M * TPB;
+    DLayer *lay = reinterpret_cast<DLayer *>(xch + 10 * Cfg::NW);
+    for (int q = threadIdx.x; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
+        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
+    __syncthreads();
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const size_t rec = (size_t)p.batch * (size_t)p.nprobes;
+    for (int k = 0; k < p.nsteps; ++k) {
+        const long long s = p.step0 + k;
+        double inv_tau, amp;
+        dev_schedule(p.sched, s, inv_tau, amp);
+        const double *Told = (k & 1) ? p.Tnew : p.Told;
+        double *Tnew = (k & 1) ? const_cast<double *>(p.Told) : p.Tnew;
+        // probe record of this step: records are appended while the ring has room (the host mirrors
+        // this arithmetic to count written and dropped records)
+        double *probe_out = nullptr;
+        if (p.nprobes > 0 && (s + 1) % p.probe_every == 0) {
+            const long long r = p.rec0 + ((s + 1) / p.probe_every - p.step0 / p.probe_every - 1);
+            if ((size_t)(r + 1) * rec <= p.probe_cap) probe_out = p.probe_base + (size_t)r * rec;
+        }
+        line_step<M, G, true>(p, Told, Tnew, inv_tau, amp, probe_out, st, xch, lay);
+        grid.sync();
     }
 }
 

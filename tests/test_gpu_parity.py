@@ -612,3 +612,39 @@ def test_no_write_outside_the_callers_buffers(bd, case, monkeypatch):
     pg, dropped = sim.probes()
     assert pg.shape[0] == 3 and dropped == 11 // s["probe_every"] - 3 and sim.guards_intact()
     sim.close()
+
+
+@pytest.mark.parametrize("nr,nz,batch", [(64, 64, 1), (13, 11, 2), (96, 40, 3), (512, 40, 1)])
+def test_persistent_multi_step_launch_equals_single_steps(bd, nr, nz, batch, monkeypatch):
+    """heat_step(n) on the line kernel is ONE cooperative launch with the schedule, the level swap and the
+    probe slots on the device.  It must give bitwise what n single-step launches give
+    (field, probe records, dropped count, step index) -- across sub-steps, switch-off, an odd number of
+    steps and a probe ring that overflows -- and both must match the oracle."""
+    monkeypatch.setenv("HEAT_KERNEL", "line")
+    if nr == 13:
+        s = I.random_spec(5, nr=nr, nz=nz, batch=batch)
+        s["dt"] = 0.7 * bd.heat_stable_dt(s)
+    else:
+        s = with_dt(bd, I.config(3 if batch > 1 else 2, nr=nr, nz=nz, batch=batch) if nr != 64 else I.config(0))
+    if s["probes"]:
+        s["probe_every"] = 3
+    a, b = bd.HeatSim(s, probe_records=40), bd.HeatSim(s, probe_records=40)
+    orc = oracle_cls()(s)
+    before = a.launch_count
+    a.step(151)                                  # one launch
+    assert a.launch_count == before + 1
+    for _ in range(151):
+        b.step(1)                                # 151 launches
+    assert a.step_index == b.step_index == 151
+    assert np.array_equal(a.fields(), b.fields())
+    a.step(2); b.step(1); b.step(1)
+    assert np.array_equal(a.fields(), b.fields())
+    pa, da = a.probes()
+    pb, db = b.probes()
+    assert np.array_equal(pa, pb) and da == db
+    orc.step(153)
+    compare(a, orc)
+    po = orc.probes()
+    if s["probes"]:
+        assert pa.shape[0] == 40 and da == 153 // 3 - 40 and np.max(np.abs(pa - po[:40])) <= TOL
+    a.close(); b.close()
