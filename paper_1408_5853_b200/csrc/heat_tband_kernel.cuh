@@ -540,7 +540,11 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                     me.c = -sal * Pw * r;
                     me.d = fma(sal, Qw, sbe) * r;
                     Row3 s3 = pcr_combine(me, l30, true, nx, has_next);
-                    s3 = pcr_segment_rolled<WL>(s3, s, 0, WL - 1);
+                    // the separators are 512 rows apart: on diagonally dominant lines their mutual couplings
+                    // have decayed far below rounding (|a|, |c| < 2^-80 means a dropped term is below
+                    // 1e-24 |y|, i.e. < 1e-9 ulp), and then x = d already; otherwise PCR over WL lanes
+                    if (__any_sync(FULL, in3 && (fabs(s3.a) > 8.271806125530277e-25 || fabs(s3.c) > 8.271806125530277e-25)))
+                        s3 = pcr_segment_rolled<WL>(s3, s, 0, WL - 1);
                     if (in3) sts64(ysl + 8u * (uint32_t)lane, s3.d);
                     __syncwarp();
                     if (lane == 0) asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(ybar_a + 8u * pubpar) : "memory");

@@ -648,3 +648,23 @@ def test_persistent_multi_step_launch_equals_single_steps(bd, nr, nz, batch, mon
     if s["probes"]:
         assert pa.shape[0] == 40 and da == 153 // 3 - 40 and np.max(np.abs(pa - po[:40])) <= TOL
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("nr,nw", [(2048, 4), (8192, 16), (8192, 4)])
+def test_tband_with_strongly_coupled_separators(bd, nr, nw, monkeypatch):
+    """The tband kernel skips the PCR over the separator rows when their mutual couplings are below
+    2^-80 (the BASELINE-shaped grids, eta = 10 h).  On a thin grid (L/R = 10 with nz = 10: eta ~ 2000 h)
+    the line systems are barely diagonally dominant, the separators 512 rows apart stay coupled at
+    O(1) and the full separator solve runs.  These systems are ill-conditioned, so the bar is the
+    measured rounding floor: |GPU - long double| <= 3 |fp64 oracle - long double|."""
+    monkeypatch.setenv("HEAT_TBAND_NW", str(nw))
+    s = with_dt(bd, I.config(2, nr=nr, nz=10))
+    sim, o64, o80 = bd.HeatSim(s), oracle_cls()(s, variant="omp"), oracle_cls()(s, variant="long")
+    assert sim.kernel_name.startswith(f"tband<WL={nr // 512},NW={nw},"), sim.kernel_name
+    sim.step(25); o64.step(25); o80.step(25)
+    ref = o80.field(0)
+    floor = float(np.max(np.abs(o64.field(0) - ref)))
+    gpu = float(np.max(np.abs(sim.field(0) - ref)))
+    print(f"nr = {nr}: |fp64 oracle - long double| = {floor:.3e} K, |GPU - long double| = {gpu:.3e} K")
+    assert gpu <= 3.0 * floor + 1e-12
+    sim.close()
