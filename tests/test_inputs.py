@@ -89,3 +89,29 @@ def test_paper_device_runs_on_the_oracle():
     T = o.field()
     assert np.all(np.isfinite(T)) and T.min() >= 4.2 - 1e-9 and T.max() > 6.0     # the heater warms up during the 1 ms pulse
     assert np.all(T[-1] == 4.2)                                                   # Dirichlet terminal at z_max
+
+
+def test_design_sweep_host_logic():
+    """the source-control loop's host side (no device): the objective prefers coverage
+    only while the surface cools below T_crit between pulses, the first generation contains the
+    paper's design point, refinement keeps the best member and stays inside the admissible box, and
+    every member's descriptor is accepted by the library (moving interface, Q0 from its own S_2)."""
+    from paper_1408_5853_b200 import binding, design_sweep as D
+    assert D.objective(0.75, 40.0, 42.2) == 0.75 and D.objective(0.9, 44.0, 42.2) < 0
+    rng = np.random.Generator(np.random.PCG64(1))
+    i0, th = D.first_generation(8, rng)
+    assert i0[0] == 0.363 and th[0] == 100 and len(set(th.tolist())) > 4
+    assert i0.min() >= D.I0_RANGE[0] and i0.max() <= D.I0_RANGE[1]
+    J = np.array([0.1, 0.5, -0.2, 0.3, 0.0, 0.2, 0.4, 0.45])
+    ni, nt = D.next_generation(i0, th, J, 0, 0.5, rng)
+    assert ni[0] == i0[1] and nt[0] == th[1]
+    assert np.all(np.abs(ni - i0[1]) <= 0.25 * (D.I0_RANGE[1] - D.I0_RANGE[0]) + 1e-12)
+    assert nt.min() >= D.THICK_RANGE[0] and nt.max() <= D.THICK_RANGE[1]
+    s = D.device_batch(i0[:3], th[:3], 41)
+    assert s["batch"] == 3 and s["seg_layer"].shape == (3, 630)
+    ref = I.paper_device(41)
+    assert np.array_equal(s["seg_layer"][0], ref["seg_layer"][0]) and s["Q0"][0] == pytest.approx(ref["Q0"][0], rel=1e-12)
+    for b in range(3):
+        nodes = np.flatnonzero(np.diff(s["seg_layer"][b].astype(int))) + 1
+        assert nodes[0] == 420 and nodes[2] == 620 and nodes[1] == 620 - th[b]
+    assert binding.heat_workspace_bytes(s) > 0
