@@ -2,16 +2,19 @@
 // band kernel (heat_wband_kernel.cuh) with the sweep coefficients parked in TENSOR MEMORY.
 //
 // Why: heat_wband_kernel is purely latency-bound -- its throughput on 8192 x 8192 is proportional
-// to the warps per SM (4 warps: 60, 6: 88, 8: 113 GCUPS, profiles/r02_wband_scaling.md) -- and the
+// to the warps per SM (4 warps: 60, 6: 88, 8: 113 GCUPS, profiles/r02_tband_summary.md) -- and the
 // 96 registers that hold (alpha, beta, gamma) of a thread's 16 rows between the forward sweep (12)
 // and the back substitution (14) cap it at 8 warps per SM.  Blackwell's tensor memory gives every
 // thread of a warp a private 512-byte strip (its lane x 128 columns of 32 bits): exactly 16 rows x
 // (alpha, beta, gamma, face flux).  With those parked there (tcgen05.st during the sweep,
 // tcgen05.ld during the back substitution) the kernel needs <= 128 registers and three 4 KB line
 // slots per warp, so 16 warps = 8192 nodes x 16 B of state are in flight per SM: a whole line of
-// the large grid, in four independent CTAs whose waits overlap.
-// Everything else (one branch-free row loop, per-warp TMA pipelines, separator exchange by
-// st.async + mbarrier) is as in heat_wband_kernel.cuh; same coverage, same arithmetic.
+// the large grid.
+// Further differences from heat_wband_kernel.cuh: the row loop is rolled over groups of four rows
+// with a plain and a general body chosen per warp and group (tgroup), one duty warp per CTA solves
+// the separator rows (and skips their PCR when it cannot change the result), a whole line sits in
+// one CTA where it fits (nr = 8192: 16 warps, no cluster).  Per-warp TMA pipelines and the
+// separator exchange by st.async + mbarrier are as there; same coverage, same arithmetic.
 // "P:Lnnn" cites a line of the paper text; readings G1..G22 are listed in DESIGN.md.
 #pragma once
 #include <cuda.h>

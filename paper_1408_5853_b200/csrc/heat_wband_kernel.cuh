@@ -2,7 +2,7 @@
 // "warp-autonomous band kernel" (same arithmetic contract as
 // heat_band_kernel.cuh, whose row formulas, sweep and PCR helpers it reuses).
 //
-// What the phase clocks of the band kernel showed on 8192 x 8192 (profiles/r02_phase_clocks.md):
+// What the phase clocks of the band kernel showed on 8192 x 8192:
 // the 8-row sweep of a warp is already bound by the FP64 pipe, but a line takes ~8300 cycles
 // because (i) warps that hold an interface node or an r boundary run branchy code at half speed
 // and every warp of the 4-SM cluster waits for them, (ii) the reduced system (PCR over the
