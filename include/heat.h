@@ -148,6 +148,14 @@ heat_status heat_get_field(heat_ctx *c, int32_t b, double *dst, int32_t dst_is_d
 heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t src_is_device,
                            int64_t step_index, void *cuda_stream);
 
+/* One z-line (nr doubles, r fastest) of the current level of batch member b: read it, or overwrite it
+ * in both levels.  These are what a z-slab multi-GPU run exchanges after every step (SURVEY 8(e):
+ * P:L125 couples line j only to lines j -+ 1 of the old level): a slab's halo line is a Dirichlet z
+ * line, which no step ever writes (G17), refreshed with the neighbour's edge line.  Asynchronous on
+ * cuda_stream for device pointers; a host pointer synchronises the stream. */
+heat_status heat_get_line(heat_ctx *c, int32_t b, int32_t j, double *dst, int32_t dst_is_device, void *cuda_stream);
+heat_status heat_set_line(heat_ctx *c, int32_t b, int32_t j, const double *src, int32_t src_is_device, void *cuda_stream);
+
 /* Drain the probe trace: synchronise cuda_stream, copy up to max doubles (whole records of
  * batch*nprobes doubles, order [record][batch][probe]) to dst_host, and rewind the device
  * buffer.  *n_written = doubles copied; *n_dropped (optional) = records lost to overflow. */

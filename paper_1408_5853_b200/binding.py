@@ -23,7 +23,7 @@ STATUS_NAMES = {0: "HEAT_OK", 1: "HEAT_EINVAL", 2: "HEAT_ENOMEM", 3: "HEAT_ECUDA
 
 EXPORTS = [
     "heat_workspace_bytes", "heat_stable_dt", "heat_create", "heat_step", "heat_get_field",
-    "heat_set_field", "heat_probe", "heat_schedule", "heat_step_index", "heat_launch_count",
+    "heat_set_field", "heat_get_line", "heat_set_line", "heat_probe", "heat_schedule", "heat_step_index", "heat_launch_count",
     "heat_kernel_name", "heat_last_error", "heat_destroy", "heat_fp64_peak", "heat_fp64_peak_scratch_bytes",
 ]
 
@@ -103,6 +103,10 @@ def lib():
         L.heat_last_error.argtypes = [vp]
         L.heat_destroy.restype = None
         L.heat_destroy.argtypes = [vp]
+        L.heat_get_line.restype = C.c_int
+        L.heat_get_line.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int32, vp]
+        L.heat_set_line.restype = C.c_int
+        L.heat_set_line.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int32, vp]
         L.heat_fp64_peak.restype = C.c_int
         L.heat_fp64_peak.argtypes = [i64, vp, C.c_size_t, vp, C.POINTER(dbl)]
         L.heat_fp64_peak_scratch_bytes.restype = C.c_size_t
@@ -315,6 +319,21 @@ class HeatSim:
         else:
             T = np.ascontiguousarray(T, dtype=np.float64).reshape(self.nz, self.nr)
             self._check(self._L.heat_set_field(self._h, int(b), C.c_void_p(T.ctypes.data), 0, int(step_index), self._s()))
+
+    def get_line(self, b, j):
+        """heat_get_line into a fresh device tensor [nr] (asynchronous)."""
+        out = self._torch.empty(self.nr, dtype=self._torch.float64, device=self.field_a.device)
+        self._check(self._L.heat_get_line(self._h, int(b), int(j), C.c_void_p(out.data_ptr()), 1, self._s()))
+        return out
+
+    def set_line(self, b, j, values):
+        """heat_set_line from a device tensor or a host array of nr doubles."""
+        if hasattr(values, "is_cuda") and values.is_cuda:
+            assert values.is_contiguous() and values.dtype == self._torch.float64 and values.numel() == self.nr
+            self._check(self._L.heat_set_line(self._h, int(b), int(j), C.c_void_p(values.data_ptr()), 1, self._s()))
+        else:
+            v = np.ascontiguousarray(np.asarray(values, dtype=np.float64).reshape(self.nr))
+            self._check(self._L.heat_set_line(self._h, int(b), int(j), C.c_void_p(v.ctypes.data), 0, self._s()))
 
     def probes(self, max_records=None):
         """heat_probe: drain the trace, shape [records, batch, nprobes]; also returns drops."""

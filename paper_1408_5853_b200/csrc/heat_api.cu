@@ -1027,6 +1027,8 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         wp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
         wp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
         wp.rpl = nr / 16; wp.BL = best_BL; wp.bands_per_member = bpm; wp.total_bands = (int)bands;
+        wp.stagger = 0;
+        if (const char *es = getenv("HEAT_STAGGER")) wp.stagger = atoi(es);
     }
 
     KParams &k = c->kp;
@@ -1199,6 +1201,29 @@ heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t sr
     CUDA_TRY(&c->err, cudaMemcpyAsync(c->nxt + (size_t)b * n, c->cur + (size_t)b * n, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
     if (!src_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
     c->step = step_index;
+    return HEAT_OK;
+}
+
+heat_status heat_get_line(heat_ctx *c, int32_t b, int32_t j, double *dst, int32_t dst_is_device, void *cuda_stream)
+{
+    if (!c || !dst || b < 0 || b >= c->batch || j < 0 || j >= c->nz) { if (c) set_err(&c->err, "heat_get_line: bad arguments"); return HEAT_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t off = ((size_t)b * c->nz + (size_t)j) * (size_t)c->nr;
+    CUDA_TRY(&c->err, cudaMemcpyAsync(dst, c->cur + off, sizeof(double) * (size_t)c->nr,
+                                      dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (!dst_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
+    return HEAT_OK;
+}
+
+heat_status heat_set_line(heat_ctx *c, int32_t b, int32_t j, const double *src, int32_t src_is_device, void *cuda_stream)
+{
+    if (!c || !src || b < 0 || b >= c->batch || j < 0 || j >= c->nz) { if (c) set_err(&c->err, "heat_set_line: bad arguments"); return HEAT_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t off = ((size_t)b * c->nz + (size_t)j) * (size_t)c->nr;
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CUDA_TRY(&c->err, cudaMemcpyAsync(c->cur + off, src, sizeof(double) * (size_t)c->nr, kind, st));
+    CUDA_TRY(&c->err, cudaMemcpyAsync(c->nxt + off, c->cur + off, sizeof(double) * (size_t)c->nr, cudaMemcpyDeviceToDevice, st));
+    if (!src_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
     return HEAT_OK;
 }
 

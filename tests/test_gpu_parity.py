@@ -668,3 +668,28 @@ def test_tband_with_strongly_coupled_separators(bd, nr, nw, monkeypatch):
     print(f"nr = {nr}: |fp64 oracle - long double| = {floor:.3e} K, |GPU - long double| = {gpu:.3e} K")
     assert gpu <= 3.0 * floor + 1e-12
     sim.close()
+
+
+@pytest.mark.parametrize("nr,nz,world", [(512, 40, 2), (1024, 23, 3), (96, 30, 2)])
+def test_zslab_run_equals_the_single_gpu_run_bitwise(bd, nr, nz, world):
+    """the z-slab sharding (paper_1408_5853_b200/zslab.py) on ONE GPU -- every slab is
+    its own library context with Dirichlet halo lines, the contexts are stepped in turn and exchange one
+    edge line per neighbour and step through heat_get_line / heat_set_line (device to device; no
+    kernel waits on another).  The gathered field must be bitwise the single-context field, across
+    sub-steps and switch-off, for the tband and the line kernel."""
+    from paper_1408_5853_b200 import zslab as Z
+    s = with_dt(bd, I.config(2, nr=nr, nz=nz))
+    one = bd.HeatSim(s)
+    slabs = [bd.HeatSim(Z.slab_spec(s, r, world)) for r in range(world)]
+    assert all(q.kernel_name == one.kernel_name for q in slabs)
+    for n in (1, 60, 90):
+        one.step(n)
+        Z.step_slabs_in_one_process(slabs, nz, n)
+        got = Z.gather_field([q.fields() for q in slabs], nz)
+        assert np.array_equal(got, one.fields())
+    orc = oracle_cls()(s)
+    orc.step(151)
+    compare(one, orc)
+    one.close()
+    for q in slabs:
+        q.close()
