@@ -152,8 +152,8 @@ __device__ __forceinline__ TRowCoef<DEGK> trow_coef(uint32_t a)
 // The caller picks the body per warp and group (warp-uniform), so the common case runs the plain body
 // and the instruction cache holds four rows of each kind instead of sixteen.
 template <int DEGK, bool SQ, bool GEN>
-__device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, const WCoef<DEGK> &c, SweepState &st, TSweepOut &o,
-                                       double2 &tl, double lamA_if, double lamB_if)
+__device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &c, SweepState &st, TSweepOut &o,
+                                       double2 &tl, double lamA_if, double lamB_if, uint32_t spmask)
 {
     TRaw8 fraw;
     tmem_ld8(A.tm + 96u + 8u * (uint32_t)g, fraw); // the four lower face fluxes of the group
@@ -179,18 +179,26 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, const WCoef<D
         const uint32_t k = 4u * (uint32_t)g + (uint32_t)r;
         const double fi = fig + (double)r;
         double cfR, w, f, alk;
-        if (!GEN) {
+        // GEN: only the rows that are special in SOME lane of the warp (warp-uniform bit of spmask) take
+        // the general code; the thread that holds the interface row switches its coefficients to layer B
+        // there (the face i* + 1/2 already belongs to layer B, G14) and keeps them for the rest of the line
+        if (!GEN || !((spmask >> k) & 1u)) {
             wrow2<DEGK, SQ>(c.K, c.Ct, c.qs, c.sq, T, Tr, Tu, fD[r], fi, fi, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
             sweep_row(st, cfR, w, f, alk);
         } else {
-            const bool isB = (k >= ksw), isif = (k == ksw);
-            const TRowCoef<DEGK> cr = trow_coef<DEGK>(isB ? A.layB : A.layA);
-            const double qs = isB ? A.qsB : A.qsA;
-            const bool sq = isB ? A.sqB : A.sqA;
+            const bool isif = (k == ksw);
+            if (isif) {
+                const TRowCoef<DEGK> cb = trow_coef<DEGK>(A.layB);
+#pragma unroll
+                for (int n = 0; n <= DEGK; ++n) c.K[n] = cb.K[n];
+#pragma unroll
+                for (int n = 0; n < 4; ++n) c.Ct[n] = cb.Ct[n];
+                c.qs = A.qsB; c.sq = A.sqB;
+            }
             double fie = fi;
             if (r == 3) fie = lastg ? A.fie15 : fie;
             fie = isif ? 0.0 : fie;
-            wrow2<DEGK, SQ>(cr.K, cr.Ct, qs, sq, T, Tr, Tu, fD[r], fi, fie, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
+            wrow2<DEGK, SQ>(c.K, c.Ct, c.qs, c.sq, T, Tr, Tu, fD[r], fi, fie, A.g0, A.ezp, A.ezm, cfR, w, f, fu[r]);
             // (18) times h: -lam_A x_{i-1} + (lam_A + lam_B) x_i - lam_B x_{i+1} = 0 (new level, G7)
             double cfL_use = isif ? lamA_if : st.cfL;
             double cfR_use = isif ? lamB_if : cfR;
@@ -231,7 +239,7 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, const WCoef<D
 // gamma) and the new face fluxes of a group go to tensor memory, the prefix products for the reduced
 // row are carried along.  genmask: bit g set = group g of this warp needs the general body.
 template <int DEGK, bool SQ>
-__device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, WCoef<DEGK> &c, uint32_t genmask)
+__device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, WCoef<DEGK> &c, uint32_t genmask, uint32_t spmask)
 {
     SweepState st;
     st.om = 1.0; st.be = 0.0; st.gm = 1.0;
@@ -255,20 +263,8 @@ __device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, WCoef<DEGK> &
     st.cfL = wlam<DEGK, SQ>(c.K, c.sq, A.hl + tl.x) * A.gl0; // face i0 - 1/2
 #pragma unroll 1
     for (int g = 0; g < 4; ++g) {
-        if (!((genmask >> g) & 1u)) {
-            tgroup<DEGK, SQ, false>(A, g, c, st, o, tl, lamA_if, lamB_if);
-        } else {
-            tgroup<DEGK, SQ, true>(A, g, c, st, o, tl, lamA_if, lamB_if);
-            // behind its interface row the thread is in layer B
-            if (A.ks >= 0 && (A.ks >> 2) == g) {
-                const TRowCoef<DEGK> cb = trow_coef<DEGK>(A.layB);
-#pragma unroll
-                for (int n = 0; n <= DEGK; ++n) c.K[n] = cb.K[n];
-#pragma unroll
-                for (int n = 0; n < 4; ++n) c.Ct[n] = cb.Ct[n];
-                c.qs = A.qsB; c.sq = A.sqB;
-            }
-        }
+        if (!((genmask >> g) & 1u)) tgroup<DEGK, SQ, false>(A, g, c, st, o, tl, lamA_if, lamB_if, 0u);
+        else tgroup<DEGK, SQ, true>(A, g, c, st, o, tl, lamA_if, lamB_if, spmask);
     }
     return o;
 }
@@ -407,6 +403,8 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
         // groups of four rows that need the general body: the one with the interface row, the first
         // group of the first chunk and the last group of the last chunk of the line
         const uint32_t genmask = __reduce_or_sync(FULL, (ks >= 0 ? (1u << (ks >> 2)) : 0u) | (first ? 1u : 0u) | (last ? 8u : 0u));
+        // rows (0 .. 15) that are an interface row or an r-boundary row in some lane of this warp
+        const uint32_t spmask = __reduce_or_sync(FULL, (ks >= 0 ? (1u << ks) : 0u) | (first ? 1u : 0u) | (last ? (1u << 15) : 0u));
 
         if (lane == 0) {
             const uint32_t npre = (uint32_t)min(NS, nl + 2);
@@ -471,7 +469,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
 
             // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 16 rows
             A.sc = sc; A.su = su; A.hl = hl; A.hr = hr; A.fi0 = fi0; A.ezp = ezp; A.ezm = ezm;
-            const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, c, genmask) : tsweep16<DEGK, false>(A, c, genmask);
+            const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, c, genmask, spmask) : tsweep16<DEGK, false>(A, c, genmask, spmask);
             tmem_wait_st();
             // the slot of line j - 1 has been stored (its TMA store was issued a whole sweep ago): refill it
             if (lane == 0 && L >= 1 && L + NS <= nl + 1) { tma_wait_read0(); issue_load((uint32_t)(L + NS)); }
