@@ -67,9 +67,9 @@ __device__ __forceinline__ Row3 pcr_segment(Row3 row, int lane, int lo, int hi)
     return row;
 }
 
-template <int M, int G>
+template <int M, int G, int TPBMIN = 256>
 struct LineCfg {
-    static constexpr int TPB = (G > 256) ? G : 256;
+    static constexpr int TPB = (G > TPBMIN) ? G : TPBMIN;
     static constexpr int LPB = TPB / G;               // lines in flight per block
     static constexpr int WG = (G >= 32) ? G / 32 : 1; // warps per group
     static constexpr bool MULTI = (G > 32);
@@ -84,15 +84,21 @@ struct LineCfg {
 
 // field loads: read-only path for a one-step launch; for the persistent multi-step kernel the level
 // read in step k was written in step k-1 of the same launch, so it must come from L2 (ld.global.cg)
-template <bool COH, typename T>
-__device__ __forceinline__ T ldT(const T *ptr) { return COH ? __ldcg(ptr) : __ldg(ptr); }
+// COH = 2: the field lives in shared memory (single-CTA kernel): plain loads through generic pointers
+template <int COH, typename T>
+__device__ __forceinline__ T ldT(const T *ptr)
+{
+    if (COH == 0) return __ldg(ptr);
+    if (COH == 1) return __ldcg(ptr);
+    return *ptr;
+}
 
 // One solver step of the lines this CTA owns (grid-stride over groups of LPB lines).
-template <int M, int G, bool COH>
+template <int M, int G, int COH, int TPBMIN = 256>
 __device__ __forceinline__ void line_step(const KParams &p, const double *Told, double *Tnew, double inv_tau_k, double amp_k,
                                           double *probe_out, double *st, double *xch, const DLayer *lay)
 {
-    using Cfg = LineCfg<M, G>;
+    using Cfg = LineCfg<M, G, TPBMIN>;
     constexpr int TPB = Cfg::TPB;
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -356,7 +362,7 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_kernel(const __g
     for (int q = threadIdx.x; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
         reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
     __syncthreads();
-    line_step<M, G, false>(p, p.Told, p.Tnew, p.inv_tau, p.amp, p.probe_out, st, xch, lay);
+    line_step<M, G, 0>(p, p.Told, p.Tnew, p.inv_tau, p.amp, p.probe_out, st, xch, lay);
 }
 
 // (tau_k, amplitude_k) of solver step s from integer counters only: (4) P:L79 and (22) + procedure
@@ -405,9 +411,54 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_persist_kernel(c
             const long long r = p.rec0 + ((s + 1) / p.probe_every - p.step0 / p.probe_every - 1);
             if ((size_t)(r + 1) * rec <= p.probe_cap) probe_out = p.probe_base + (size_t)r * rec;
         }
-        line_step<M, G, true>(p, Told, Tnew, inv_tau, amp, probe_out, st, xch, lay);
+        line_step<M, G, 1>(p, Told, Tnew, inv_tau, amp, probe_out, st, xch, lay);
         grid.sync();
     }
+}
+
+// Single-CTA version for problems whose two levels fit the shared memory of one SM (configs[0]:
+// 64 x 64 nodes = 32 KB per level): the field is copied in once, p.nsteps solver steps run on it with
+// a __syncthreads between them (schedule, level swap and probe slots on the device as in the
+// persistent kernel), and the final level is copied out.  1024 threads = every line of the grid at
+// once.  The step function is the same line_step, so the arithmetic and the result are bitwise those
+// of the one-step launches.
+template <int M, int G>
+__global__ void __launch_bounds__(1024, 1) heat_line_small_kernel(const __grid_constant__ KParams p)
+{
+    using Cfg = LineCfg<M, G, 1024>;
+    constexpr int TPB = Cfg::TPB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *st = reinterpret_cast<double *>(smem_raw); // [3][M][TPB]
+    double *xch = st + 3 * M * TPB;                    // [10][NW]
+    DLayer *lay = reinterpret_cast<DLayer *>(xch + 10 * Cfg::NW);
+    const size_t cells = (size_t)p.batch * (size_t)p.nz * (size_t)p.nr;
+    double *lev0 = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(lay) + ((sizeof(DLayer) * (size_t)p.nlayers + 15) & ~(size_t)15));
+    double *lev1 = lev0 + cells;
+    for (int q = threadIdx.x; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
+        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
+    // both levels: the Dirichlet z lines of the "next" level are never written by a step (G17)
+    for (size_t q = threadIdx.x; q < cells; q += TPB) { lev0[q] = p.Told[q]; lev1[q] = p.Tnew[q]; }
+    __syncthreads();
+    const size_t rec = (size_t)p.batch * (size_t)p.nprobes;
+    for (int k = 0; k < p.nsteps; ++k) {
+        const long long s = p.step0 + k;
+        double inv_tau, amp;
+        dev_schedule(p.sched, s, inv_tau, amp);
+        const double *Told = (k & 1) ? lev1 : lev0;
+        double *Tnew = (k & 1) ? lev0 : lev1;
+        double *probe_out = nullptr;
+        if (p.nprobes > 0 && (s + 1) % p.probe_every == 0) {
+            const long long r = p.rec0 + ((s + 1) / p.probe_every - p.step0 / p.probe_every - 1);
+            if ((size_t)(r + 1) * rec <= p.probe_cap) probe_out = p.probe_base + (size_t)r * rec;
+        }
+        line_step<M, G, 2, 1024>(p, Told, Tnew, inv_tau, amp, probe_out, st, xch, lay);
+        __syncthreads();
+    }
+    // after n steps the current level is lev[n & 1] and the host names it p.Tnew if n is odd, p.Told if even
+    const double *cur = (p.nsteps & 1) ? lev1 : lev0, *oth = (p.nsteps & 1) ? lev0 : lev1;
+    double *gcur = (p.nsteps & 1) ? p.Tnew : const_cast<double *>(p.Told);
+    double *goth = (p.nsteps & 1) ? const_cast<double *>(p.Told) : p.Tnew;
+    for (size_t q = threadIdx.x; q < cells; q += TPB) { gcur[q] = cur[q]; goth[q] = oth[q]; }
 }
 
 // ---------------------------------------------------------------- fp64 FMA peak probe
