@@ -1027,8 +1027,6 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         wp.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
         wp.z_hi_neumann = (d->z_hi.kind == HEAT_BC_NEUMANN0);
         wp.rpl = nr / 16; wp.BL = best_BL; wp.bands_per_member = bpm; wp.total_bands = (int)bands;
-        wp.stagger = 0;
-        if (const char *es = getenv("HEAT_STAGGER")) wp.stagger = atoi(es);
     }
 
     KParams &k = c->kp;

@@ -450,10 +450,6 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             const double ezm = __ldg(p.ezm + j), ezp = __ldg(p.ezp + j);
             asm volatile("" : "+d"(fi0)); // keep the per-row geometry out of registers across lines
             wait_seq((uint32_t)(L + 2));
-            if (p.stagger > 0) { // experiment: stagger the warps that share a scheduler
-                const long long t0 = clock64(); const long long dd = (long long)(warp >> 2) * (long long)p.stagger;
-                while (clock64() - t0 < dd) {}
-            }
 
             // ---- the two r neighbours of the thread's 16 nodes at line j
             double hl, hr;

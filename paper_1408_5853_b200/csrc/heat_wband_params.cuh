@@ -44,7 +44,6 @@ struct WParams {
     int rpl;  // tensor rows (16 doubles) per line = threads per line
     int BL;   // lines per band
     int bands_per_member, total_bands;
-    int stagger; // experiment
 };
 
 // WL = warps per line (nr = 512 WL), NW = warps per CTA.  A line wider than a CTA spans a cluster
