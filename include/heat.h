@@ -192,6 +192,29 @@ void heat_destroy(heat_ctx *c);
 size_t heat_fp64_peak_scratch_bytes(void);
 heat_status heat_fp64_peak(int64_t iters, void *scratch, size_t scratch_bytes, void *cuda_stream, double *tflops);
 
+/* ---- allocation-free set-up ---------------------------------------------------------------------
+ * heat_create for callers that cannot call cudaMalloc (set-up next to CUDA graph capture, serving loops,
+ * harnesses that forbid it): the same call without the workspace arguments.  The row tables that every
+ * step kernel reads (the coefficients of rows (13), (15), (18) P:L140-192, the z factors
+ * of (11) P:L125, the law tables) live in a static device array of HEAT_STATIC_WORKSPACE_BYTES inside
+ * the library, which every GPU that loads the library holds until the process exits.  The call
+ * allocates no device memory (neither does any other call of this library: they take caller-owned
+ * buffers); field_a, field_b, probe_buf are the caller's as in heat_create.
+ *   - HEAT_ENOMEM with a message naming both sizes if heat_workspace_bytes(d) exceeds the array;
+ *     the five BASELINE.json configurations need 0.01 - 2.7 MiB (configs[3]: 2 772 992 B).
+ *   - The array is shared by every heat_create_static context of the process on that device and keeps
+ *     the previous one's contents; each call clears the part it uses before the upload.  Hence at most
+ *     ONE live heat_create_static context per device: creating a second one overwrites the tables
+ *     under the first, and calls that overlap on the GPU (a step of the first context still running
+ *     on another stream while the second is created) race.  Destroy the context, and let its work
+ *     finish, before the next heat_create_static on the same device.
+ * Everything else (heat_step, heat_get_field, heat_probe, heat_destroy ...) is used as with heat_create,
+ * and the results are bitwise those of heat_create (tests/test_zz_no_alloc.py). */
+#define HEAT_STATIC_WORKSPACE_BYTES (4u << 20)
+size_t heat_static_workspace_bytes(void);
+heat_status heat_create_static(const heat_desc *d, void *field_a, void *field_b, void *probe_buf,
+                               size_t probe_cap, void *cuda_stream, heat_ctx **out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,6 +25,7 @@ EXPORTS = [
     "heat_workspace_bytes", "heat_stable_dt", "heat_create", "heat_step", "heat_get_field",
     "heat_set_field", "heat_get_line", "heat_set_line", "heat_probe", "heat_schedule", "heat_step_index", "heat_launch_count",
     "heat_kernel_name", "heat_last_error", "heat_destroy", "heat_fp64_peak", "heat_fp64_peak_scratch_bytes",
+    "heat_create_static", "heat_static_workspace_bytes",
 ]
 
 
@@ -111,6 +112,10 @@ def lib():
         L.heat_fp64_peak.argtypes = [i64, vp, C.c_size_t, vp, C.POINTER(dbl)]
         L.heat_fp64_peak_scratch_bytes.restype = C.c_size_t
         L.heat_fp64_peak_scratch_bytes.argtypes = []
+        L.heat_create_static.restype = C.c_int
+        L.heat_create_static.argtypes = [C.POINTER(heat_desc), vp, vp, vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.heat_static_workspace_bytes.restype = C.c_size_t
+        L.heat_static_workspace_bytes.argtypes = []
         _lib = L
     return _lib
 
@@ -210,6 +215,10 @@ def heat_workspace_bytes(spec) -> int:
     return int(lib().heat_workspace_bytes(C.byref(Desc(spec, placeholder_dt=True).desc)))
 
 
+def heat_static_workspace_bytes() -> int:
+    return int(lib().heat_static_workspace_bytes())
+
+
 def heat_fp64_peak(iters=1 << 16) -> float:
     import torch
     out = C.c_double()
@@ -225,7 +234,9 @@ def heat_fp64_peak(iters=1 << 16) -> float:
 class HeatSim:
     """One simulation context on the current CUDA device: heat_create .. heat_destroy."""
 
-    def __init__(self, spec, probe_records=None, stream=None, T_init_device=None, guard=0):
+    def __init__(self, spec, probe_records=None, stream=None, T_init_device=None, guard=0, static_workspace=False):
+        """static_workspace=True: heat_create_static, i.e. the row tables go into the library's static
+        device array (no workspace is allocated; at most one such context alive per device)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("HeatSim needs a CUDA device (B200, sm_100a); there is no CPU fallback")
@@ -265,12 +276,23 @@ class HeatSim:
 
             self.field_a = banded(cells)
             self.field_b = banded(cells)
-            self._ws64 = banded((ws + 7) // 8 + 32)
-            ws_off = (-self._ws64.data_ptr()) % 256                # the workspace must be 256-byte aligned
-            self.workspace = self._ws64.view(torch.uint8)[ws_off:ws_off + ws]
+            if static_workspace:
+                self.workspace = None
+            else:
+                self._ws64 = banded((ws + 7) // 8 + 32)
+                ws_off = (-self._ws64.data_ptr()) % 256                # the workspace must be 256-byte aligned
+                self.workspace = self._ws64.view(torch.uint8)[ws_off:ws_off + ws]
             self.probe_buf = banded(self.probe_cap)
             self.probe_buf.zero_()
         h = C.c_void_p()
+        if static_workspace:
+            st = self._L.heat_create_static(C.byref(m.desc), self.field_a.data_ptr(), self.field_b.data_ptr(),
+                                            self.probe_buf.data_ptr(), self.probe_cap,
+                                            C.c_void_p(self.stream.cuda_stream), C.byref(h))
+            if st != HEAT_OK:
+                raise HeatError(st, self._L.heat_last_error(None).decode())
+            self._h = h
+            return
         st = self._L.heat_create(C.byref(m.desc), self.field_a.data_ptr(), self.field_b.data_ptr(),
                                  self.workspace.data_ptr(), ws, self.probe_buf.data_ptr(), self.probe_cap,
                                  C.c_void_p(self.stream.cuda_stream), C.byref(h))

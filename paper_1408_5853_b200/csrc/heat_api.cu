@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1273,6 +1274,63 @@ heat_status heat_fp64_peak(int64_t iters, void *scratch, size_t scratch_bytes, v
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     return HEAT_OK;
+}
+
+} // extern "C"
+
+// ---------------------------------------------------------------- allocation-free set-up
+// heat_create_static: heat_create with the row tables (the scratch every step kernel reads: ga, gc,
+// info, ezm, ezp, law tables, chunk descriptors, probe sources) in a file-scope device array instead
+// of a caller-allocated workspace, for callers that cannot call cudaMalloc (CUDA graph capture set-up,
+// serving loops, harnesses that forbid it).  Every GPU that loads the library holds the array until
+// the process exits.  The array's name is a host-side stand-in in host code, not a device address:
+// the address is looked up once per device with cudaGetSymbolAddress, with that device current.
+static __device__ __align__(256) unsigned char g_static_workspace[HEAT_STATIC_WORKSPACE_BYTES];
+
+namespace {
+constexpr int k_max_devices = 64;
+std::mutex g_static_mu;
+void *g_static_ptr[k_max_devices]; // device address of g_static_workspace per device ordinal, NULL = not looked up yet
+}
+
+extern "C" {
+
+size_t heat_static_workspace_bytes(void) { return (size_t)HEAT_STATIC_WORKSPACE_BYTES; }
+
+heat_status heat_create_static(const heat_desc *d, void *field_a, void *field_b, void *probe_buf, size_t probe_cap,
+                               void *cuda_stream, heat_ctx **out)
+{
+    if (out) *out = nullptr;
+    if (!out) { set_err(nullptr, "out is NULL"); return HEAT_EINVAL; }
+    heat_status vs = validate(d, nullptr);
+    if (vs != HEAT_OK) return vs;
+    const size_t need = heat_workspace_bytes(d);
+    if (need == 0) { set_err(nullptr, "no kernel variant covers nr = %d", d->nr); return HEAT_EINVAL; }
+    if (need > (size_t)HEAT_STATIC_WORKSPACE_BYTES) {
+        set_err(nullptr, "heat_create_static: this problem needs %zu bytes of workspace, the static array holds %zu "
+                         "(HEAT_STATIC_WORKSPACE_BYTES); use heat_create with a caller-allocated workspace",
+                need, (size_t)HEAT_STATIC_WORKSPACE_BYTES);
+        return HEAT_ENOMEM;
+    }
+    int dev = 0;
+    CUDA_TRY(nullptr, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= k_max_devices) { set_err(nullptr, "heat_create_static: device ordinal %d out of range", dev); return HEAT_EINVAL; }
+    void *ptr = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        if (!g_static_ptr[dev]) {
+            void *p = nullptr;
+            CUDA_TRY(nullptr, cudaGetSymbolAddress(&p, g_static_workspace));
+            if (!p || ((uintptr_t)p & 255u)) { set_err(nullptr, "heat_create_static: bad address of the static workspace"); return HEAT_ECUDA; }
+            g_static_ptr[dev] = p;
+        }
+        ptr = g_static_ptr[dev];
+    }
+    // the array keeps the previous context's tables: clear the part this one uses, on the stream
+    // heat_create uploads on (heat_create overwrites every table it reads; this makes the state of the
+    // alignment gaps and unused tables independent of the previous call as well)
+    CUDA_TRY(nullptr, cudaMemsetAsync(ptr, 0, need, (cudaStream_t)cuda_stream));
+    return heat_create(d, field_a, field_b, ptr, (size_t)HEAT_STATIC_WORKSPACE_BYTES, probe_buf, probe_cap, cuda_stream, out);
 }
 
 } // extern "C"
