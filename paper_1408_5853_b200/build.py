@@ -23,8 +23,14 @@ HEAT_H = os.path.join(ROOT, "include", "heat.h")
 # translation unit -> the files it is built from
 UNITS = {
     "heat_api.cu": _c("heat_api.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
-                      "heat_band_params.cuh", "heat_band_variants.h", "heat_wband_params.cuh",
-                      "heat_wband_variants.h", "heat_tband_variants.h") + [HEAT_H],
+                      "heat_line_variants.h", "heat_band_params.cuh", "heat_band_variants.h",
+                      "heat_wband_params.cuh", "heat_wband_variants.h", "heat_tband_variants.h") + [HEAT_H],
+    "heat_line_a.cu": _c("heat_line_a.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                         "heat_line_variants.h"),
+    "heat_line_b.cu": _c("heat_line_b.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                         "heat_line_variants.h"),
+    "heat_tma.cu": _c("heat_tma.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
+                      "heat_line_variants.h"),
     "heat_band.cu": _c("heat_band.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",
                        "heat_band_params.cuh", "heat_band_variants.h", "heat_band_kernel.cuh"),
     "heat_wband2.cu": _c("heat_wband2.cu", "heat_device.cuh", "heat_line_kernel.cuh", "heat_tma_kernel.cuh",

@@ -15,6 +15,7 @@
 
 #include "heat_line_kernel.cuh"
 #include "heat_tma_kernel.cuh"
+#include "heat_line_variants.h"
 #include "heat_band_variants.h"
 #include "heat_wband_variants.h"
 #include "heat_tband_variants.h"
@@ -37,27 +38,9 @@ void set_err(std::string *dst, const char *fmt, ...)
 }
 
 // ---------------------------------------------------------------- kernel variants
-typedef void (*kernel_fn)(const KParams);
-struct Variant {
-    int M, G, tpb, lpb;
-    kernel_fn fn, fn_persist;
-    const char *name;
-    size_t smem_fixed; // bytes without the layer table
-};
-
-#define HEAT_VARIANT(M_, G_)                                                                      \
-    {                                                                                             \
-        M_, G_, LineCfg<M_, G_>::TPB, LineCfg<M_, G_>::LPB, heat_line_kernel<M_, G_>,             \
-            heat_line_persist_kernel<M_, G_>,                                                     \
-            "line<M=" #M_ ",G=" #G_ ">", LineCfg<M_, G_>::smem_bytes(0)                           \
-    }
-const Variant k_variants[] = {
-    HEAT_VARIANT(4, 8),    HEAT_VARIANT(4, 16),  HEAT_VARIANT(4, 32),   HEAT_VARIANT(8, 32),
-    HEAT_VARIANT(16, 32),  HEAT_VARIANT(8, 64),  HEAT_VARIANT(16, 64),  HEAT_VARIANT(8, 128),
-    HEAT_VARIANT(16, 128), HEAT_VARIANT(8, 256), HEAT_VARIANT(16, 256), HEAT_VARIANT(8, 512),
-    HEAT_VARIANT(16, 512), HEAT_VARIANT(8, 1024),
-};
-constexpr int k_nvariants = (int)(sizeof(k_variants) / sizeof(k_variants[0]));
+// (tables in heat_line_a.cu, heat_line_b.cu, heat_tma.cu: heat_line_variants.h)
+const Variant *variant_at(int v) { return v < k_nvariants_a ? &k_variants_a[v] : &k_variants_b[v - k_nvariants_a]; }
+int nvariants() { return k_nvariants_a + k_nvariants_b; }
 
 // Default choice: the largest M (fewest reduced rows per cell) whose group covers the line.
 // HEAT_VARIANT="M,G" in the environment overrides it (tuning / tests of every variant).
@@ -66,35 +49,19 @@ const Variant *pick_variant(int nr)
     if (const char *e = getenv("HEAT_VARIANT")) {
         int M = 0, G = 0;
         if (sscanf(e, "%d,%d", &M, &G) == 2)
-            for (int v = 0; v < k_nvariants; ++v)
-                if (k_variants[v].M == M && k_variants[v].G == G && M * G >= nr) return &k_variants[v];
+            for (int v = 0; v < nvariants(); ++v)
+                if (variant_at(v)->M == M && variant_at(v)->G == G && M * G >= nr) return variant_at(v);
     }
     static const int order[][2] = {{4, 8},   {4, 16},  {4, 32},   {8, 32},   {16, 32}, {16, 64},
                                    {16, 128}, {16, 256}, {16, 512}, {8, 1024}};
     for (auto &o : order)
         if (o[0] * o[1] >= nr)
-            for (int v = 0; v < k_nvariants; ++v)
-                if (k_variants[v].M == o[0] && k_variants[v].G == o[1]) return &k_variants[v];
+            for (int v = 0; v < nvariants(); ++v)
+                if (variant_at(v)->M == o[0] && variant_at(v)->G == o[1]) return variant_at(v);
     return nullptr;
 }
 
 // ---------------------------------------------------------------- TMA kernel variants
-typedef void (*tma_kernel_fn)(const TParams);
-struct TmaVariant {
-    int G, CL;
-    tma_kernel_fn fn;
-    const char *name;
-    size_t smem_fixed; // bytes without the layer table
-};
-#define HEAT_TMA_VARIANT(G_, CL_)                                                                 \
-    {                                                                                             \
-        G_, CL_, heat_tma_kernel<G_, CL_>, "tma<G=" #G_ ",CL=" #CL_ ">", TmaCfg<G_, CL_>::smem_bytes(0) \
-    }
-const TmaVariant k_tma_variants[] = {
-    HEAT_TMA_VARIANT(8, 1),   HEAT_TMA_VARIANT(16, 1),  HEAT_TMA_VARIANT(32, 1),  HEAT_TMA_VARIANT(64, 1),
-    HEAT_TMA_VARIANT(128, 1), HEAT_TMA_VARIANT(128, 2), HEAT_TMA_VARIANT(128, 4),
-};
-
 // The TMA kernel covers lines of 16*G*CL nodes exactly (nr = 128 .. 8192, powers of two);
 // every other nr, HEAT_KERNEL=line or HEAT_VARIANT in the environment select the line kernel.
 const TmaVariant *pick_tma_variant(int nr)
@@ -103,8 +70,8 @@ const TmaVariant *pick_tma_variant(int nr)
     if (const char *e = getenv("HEAT_KERNEL"))
         if (strcmp(e, "line") == 0) return nullptr;
     if (nr % 16 != 0) return nullptr;
-    for (auto &v : k_tma_variants)
-        if (16 * v.G * v.CL == nr) return &v;
+    for (int v = 0; v < k_ntma_variants; ++v)
+        if (16 * k_tma_variants[v].G * k_tma_variants[v].CL == nr) return &k_tma_variants[v];
     return nullptr;
 }
 

@@ -416,51 +416,6 @@ __global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_persist_kernel(c
     }
 }
 
-// Single-CTA version for problems whose two levels fit the shared memory of one SM (configs[0]:
-// 64 x 64 nodes = 32 KB per level): the field is copied in once, p.nsteps solver steps run on it with
-// a __syncthreads between them (schedule, level swap and probe slots on the device as in the
-// persistent kernel), and the final level is copied out.  1024 threads = every line of the grid at
-// once.  The step function is the same line_step, so the arithmetic and the result are bitwise those
-// of the one-step launches.
-template <int M, int G>
-__global__ void __launch_bounds__(1024, 1) heat_line_small_kernel(const __grid_constant__ KParams p)
-{
-    using Cfg = LineCfg<M, G, 1024>;
-    constexpr int TPB = Cfg::TPB;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double *st = reinterpret_cast<double *>(smem_raw); // [3][M][TPB]
-    double *xch = st + 3 * M * TPB;                    // [10][NW]
-    DLayer *lay = reinterpret_cast<DLayer *>(xch + 10 * Cfg::NW);
-    const size_t cells = (size_t)p.batch * (size_t)p.nz * (size_t)p.nr;
-    double *lev0 = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(lay) + ((sizeof(DLayer) * (size_t)p.nlayers + 15) & ~(size_t)15));
-    double *lev1 = lev0 + cells;
-    for (int q = threadIdx.x; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
-        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
-    // both levels: the Dirichlet z lines of the "next" level are never written by a step (G17)
-    for (size_t q = threadIdx.x; q < cells; q += TPB) { lev0[q] = p.Told[q]; lev1[q] = p.Tnew[q]; }
-    __syncthreads();
-    const size_t rec = (size_t)p.batch * (size_t)p.nprobes;
-    for (int k = 0; k < p.nsteps; ++k) {
-        const long long s = p.step0 + k;
-        double inv_tau, amp;
-        dev_schedule(p.sched, s, inv_tau, amp);
-        const double *Told = (k & 1) ? lev1 : lev0;
-        double *Tnew = (k & 1) ? lev0 : lev1;
-        double *probe_out = nullptr;
-        if (p.nprobes > 0 && (s + 1) % p.probe_every == 0) {
-            const long long r = p.rec0 + ((s + 1) / p.probe_every - p.step0 / p.probe_every - 1);
-            if ((size_t)(r + 1) * rec <= p.probe_cap) probe_out = p.probe_base + (size_t)r * rec;
-        }
-        line_step<M, G, 2, 1024>(p, Told, Tnew, inv_tau, amp, probe_out, st, xch, lay);
-        __syncthreads();
-    }
-    // after n steps the current level is lev[n & 1] and the host names it p.Tnew if n is odd, p.Told if even
-    const double *cur = (p.nsteps & 1) ? lev1 : lev0, *oth = (p.nsteps & 1) ? lev0 : lev1;
-    double *gcur = (p.nsteps & 1) ? p.Tnew : const_cast<double *>(p.Told);
-    double *goth = (p.nsteps & 1) ? const_cast<double *>(p.Told) : p.Tnew;
-    for (size_t q = threadIdx.x; q < cells; q += TPB) { gcur[q] = cur[q]; goth[q] = oth[q]; }
-}
-
 // ---------------------------------------------------------------- fp64 FMA peak probe
 static __global__ void fp64_peak_kernel(double *out, long long iters, double a, double b)
 {
