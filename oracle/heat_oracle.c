@@ -23,13 +23,17 @@
  *   G7  (18) second line is at the new level        G8  (22) exponent is negative
  *   G9  source sampled at the start of the step     G14 material belongs to r-segments
  *   G16 Neumann z-line copies its neighbour         G17 Dirichlet z-lines are never solved
+ *   G23 (variant orc_step_picard only) "iterations at each time step" P:L206 = simple iteration on
+ *       the coefficients: laws at the previous iterate, the current level where (8) has it
  *
  * Pins: tests/test_oracle_*.py (dense solve, discrete steady state, ln r, z-sine growth
  * factor, Bessel mode, lumped heating, energy identity, interface flux, schedule table,
  * tau-consistency with P:L278/L322) and, since round 2, tests/test_oracle_pins_r2.py: rows (13)
  * re-assembled in NumPy (both face modes), the face_mode-1 rule on a hand-computed line and in
- * the energy identity, probe records against the field of their step (bitwise).  Every function
- * here has a pin.  What the PAPER cannot decide (both sides take the same reading): which of the
+ * the energy identity, probe records against the field of their step (bitwise);
+ * tests/test_oracle_picard.py for orc_step_picard (bitwise the paper's step for one iteration and
+ * for T-independent laws, a NumPy residual of the rows with the laws at the previous iterate, the
+ * fixed point).  Every function here has a pin.  What the PAPER cannot decide (both sides take the same reading): which of the
  * two face rules G3 it means, and G9.
  */
 #include <math.h>
@@ -106,6 +110,7 @@ typedef struct {
     int32_t *probe_ij;
     /* state */
     real *T, *Tn;       /* two time levels, [batch][nz][nr], r fastest */
+    real *Ts;           /* iterate of the new level (orc_step_picard only; allocated on first use) */
     real *alpha, *beta; /* sweep coefficients, one line per j (nz*nr) so that lines are independent */
     int64_t step;       /* solver steps done */
     double *probe;      /* growable: batch*nprobes values per record */
@@ -177,9 +182,13 @@ void orc_schedule(const orc_ctx *c, int64_t s, double *tau, double *amp)
 /* ------------------------------------------------------------------ rows */
 
 /* Coefficients (13) P:L140-145 of a regular node (i,j), layer m, from the current level T.
- * Tl = line j, Tm = line j-1, Tp = line j+1. */
+ * Tl = line j, Tm = line j-1, Tp = line j+1.
+ * Sm, Sl, Sp: the same three lines of the field at which lambda, c_V and X are EVALUATED.  In the
+ * paper's scheme that is the current level itself (S == T: "without using iterations"); in
+ * the iterated variant (orc_step_picard below) it is the previous iterate of the new level. */
 static void regular_row(const orc_ctx *c, int b, int i, int j, int m, real tau, real amp,
                         const real *Tm, const real *Tl, const real *Tp,
+                        const real *Sm, const real *Sl, const real *Sp,
                         real *A, real *B, real *C, real *F)
 {
     const orc_layer *Lm = &c->layers[m];
@@ -194,14 +203,15 @@ static void regular_row(const orc_ctx *c, int b, int i, int j, int m, real tau, 
     real r_mh = ((real)r[i] + (real)r[i - 1]) / 2;   /* r_{i-1/2} */
     real r_ph = ((real)r[i] + (real)r[i + 1]) / 2;   /* r_{i+1/2} */
     real T_ij = Tl[i];
-    real lam_mh = face_lambda(c, &Lm->k, T_ij, Tl[i - 1]); /* lambda_{i-1/2,j} */
-    real lam_ph = face_lambda(c, &Lm->k, T_ij, Tl[i + 1]); /* lambda_{i+1/2,j} */
-    real lam_jm = face_lambda(c, &Lm->k, T_ij, Tm[i]);     /* lambda_{i,j-1/2} */
-    real lam_jp = face_lambda(c, &Lm->k, T_ij, Tp[i]);     /* lambda_{i,j+1/2} */
-    real rc = (real)Lm->rho * law_eval(&Lm->cp, T_ij);     /* rho_{i,j} c_V{i,j} */
+    real S_ij = Sl[i];
+    real lam_mh = face_lambda(c, &Lm->k, S_ij, Sl[i - 1]); /* lambda_{i-1/2,j} */
+    real lam_ph = face_lambda(c, &Lm->k, S_ij, Sl[i + 1]); /* lambda_{i+1/2,j} */
+    real lam_jm = face_lambda(c, &Lm->k, S_ij, Sm[i]);     /* lambda_{i,j-1/2} */
+    real lam_jp = face_lambda(c, &Lm->k, S_ij, Sp[i]);     /* lambda_{i,j+1/2} */
+    real rc = (real)Lm->rho * law_eval(&Lm->cp, S_ij);     /* rho_{i,j} c_V{i,j} */
     real X = 0;
     if (Lm->is_heater)                                     /* X_{i,j} = X_m(T_{i,j}), (2)-(4) */
-        X = (real)c->Q0[b] * law_eval(&Lm->src_shape, T_ij) * amp;
+        X = (real)c->Q0[b] * law_eval(&Lm->src_shape, S_ij) * amp;
     /* Lambda_j[T_{i,j}], eq. (11) */
     real Lj = (1 / etabar) * (lam_jp * (Tp[i] - T_ij) / eta_jp - lam_jm * (T_ij - Tm[i]) / eta_j);
     *A = -r_mh * lam_mh / (r_i * hbar * h_i);
@@ -212,10 +222,11 @@ static void regular_row(const orc_ctx *c, int b, int i, int j, int m, real tau, 
 
 /* One line j of batch member b: forward sweep (12),(16),(20), then (17) and back sweep (14). */
 static void line_solve(const orc_ctx *c, int b, int j, real tau, real amp,
-                       const real *T, real *Tn, real *alpha, real *beta)
+                       const real *T, const real *S, real *Tn, real *alpha, real *beta)
 {
     int nr = c->nr, N = nr - 1;
     const real *Tm = T + (size_t)(j - 1) * nr, *Tl = T + (size_t)j * nr, *Tp = T + (size_t)(j + 1) * nr;
+    const real *Sm = S + (size_t)(j - 1) * nr, *Sl = S + (size_t)j * nr, *Sp = S + (size_t)(j + 1) * nr;
     real *out = Tn + (size_t)j * nr;
     const uint8_t *seg = c->seg_layer + (size_t)b * (nr - 1);
     const double *r = c->r;
@@ -232,8 +243,8 @@ static void line_solve(const orc_ctx *c, int b, int j, real tau, real amp,
         int m = seg[i - 1], m1 = seg[i];
         if (m != m1) {
             /* interface node i*, eq. (20), lambda* = lambda(T_{i*,j}) P:L183 */
-            real lam_m = law_eval(&c->layers[m].k, Tl[i]);
-            real lam_m1 = law_eval(&c->layers[m1].k, Tl[i]);
+            real lam_m = law_eval(&c->layers[m].k, Sl[i]);
+            real lam_m1 = law_eval(&c->layers[m1].k, Sl[i]);
             real h_i = (real)r[i] - (real)r[i - 1];
             real h_ip = (real)r[i + 1] - (real)r[i];
             real den = lam_m1 * h_i + lam_m * h_ip * (1 - alpha[i - 1]);
@@ -241,7 +252,7 @@ static void line_solve(const orc_ctx *c, int b, int j, real tau, real amp,
             beta[i] = lam_m * h_ip * beta[i - 1] / den;
         } else {
             real A, B, C, F;
-            regular_row(c, b, i, j, m, tau, amp, Tm, Tl, Tp, &A, &B, &C, &F);
+            regular_row(c, b, i, j, m, tau, amp, Tm, Tl, Tp, Sm, Sl, Sp, &A, &B, &C, &F);
             /* (12) P:L133-136 */
             real den = B + A * alpha[i - 1];
             alpha[i] = -C / den;
@@ -291,7 +302,7 @@ void orc_destroy(orc_ctx *c)
 {
     if (!c) return;
     free(c->r); free(c->z); free(c->layers); free(c->seg_layer); free(c->Q0);
-    free(c->probe_ij); free(c->T); free(c->Tn); free(c->alpha); free(c->beta); free(c->probe);
+    free(c->probe_ij); free(c->T); free(c->Tn); free(c->Ts); free(c->alpha); free(c->beta); free(c->probe);
     free(c);
 }
 
@@ -382,7 +393,7 @@ void orc_step(orc_ctx *c, int64_t n)
 #pragma omp parallel for schedule(static)
 #endif
             for (int j = 1; j <= M - 1; ++j)
-                line_solve(c, b, j, tau, amp, T, Tn, c->alpha + (size_t)j * nr, c->beta + (size_t)j * nr);
+                line_solve(c, b, j, tau, amp, T, T, Tn, c->alpha + (size_t)j * nr, c->beta + (size_t)j * nr);
             /* z boundaries (G16, G17; "constructed in a similar way" P:L164) */
             for (int i = 0; i < nr; ++i) {
                 Tn[i] = (c->z_lo.kind == ORC_BC_DIRICHLET) ? T[i] : Tn[(size_t)1 * nr + i];
@@ -391,6 +402,52 @@ void orc_step(orc_ctx *c, int64_t n)
             }
         }
         real *t = c->T; c->T = c->Tn; c->Tn = t; /* swap levels */
+        c->step += 1;
+        if (c->nprobes > 0 && c->step % c->probe_every == 0) append_probes(c);
+    }
+}
+
+/* Variant, not the paper's scheme: "for implicit difference schema with
+ * coefficients depending on the sought-after function (temperature), one needs to make iterations
+ * for evaluation of temperature at each time step" -- which the paper avoids.
+ * Simple (Picard) iteration on the coefficients, reading G23: T^(0) = T; T^(s+1) solves (8)-(20) with
+ * every lambda, c_V and X evaluated at T^(s) instead of T, while T itself stays where (8) has the
+ * current level: in rho c_V (T^ - T)/tau and in Lambda_j[T].  T^ = T^(iters); iters = 1 is orc_step. */
+void orc_step_picard(orc_ctx *c, int64_t n, int iters)
+{
+    int nr = c->nr, nz = c->nz, M = nz - 1;
+    size_t cells = (size_t)c->batch * nz * nr;
+    if (iters < 1) return;
+    if (!c->Ts) c->Ts = (real *)malloc(sizeof(real) * cells);
+    for (int64_t s = 0; s < n; ++s) {
+        double tau_d, amp_d;
+        orc_schedule(c, c->step, &tau_d, &amp_d);
+        real tau = (real)tau_d, amp = (real)amp_d;
+        const real *S = c->T;      /* T^(0) = T */
+        real *out = c->Tn;
+        for (int it = 0; it < iters; ++it) {
+            for (int b = 0; b < c->batch; ++b) {
+                const real *T = c->T + (size_t)b * nz * nr;
+                const real *Sb = S + (size_t)b * nz * nr;
+                real *Tn = out + (size_t)b * nz * nr;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+                for (int j = 1; j <= M - 1; ++j)
+                    line_solve(c, b, j, tau, amp, T, Sb, Tn, c->alpha + (size_t)j * nr, c->beta + (size_t)j * nr);
+                /* z boundaries of the iterate, as in orc_step */
+                for (int i = 0; i < nr; ++i) {
+                    Tn[i] = (c->z_lo.kind == ORC_BC_DIRICHLET) ? T[i] : Tn[(size_t)1 * nr + i];
+                    Tn[(size_t)M * nr + i] =
+                        (c->z_hi.kind == ORC_BC_DIRICHLET) ? T[(size_t)M * nr + i] : Tn[(size_t)(M - 1) * nr + i];
+                }
+            }
+            S = out;                                  /* the next iteration evaluates the laws here */
+            out = (out == c->Tn) ? c->Ts : c->Tn;     /* ... and writes into the other buffer */
+        }
+        /* S is T^(iters): make it the current level */
+        if (S == c->Tn) { real *t = c->T; c->T = c->Tn; c->Tn = t; }
+        else { real *t = c->T; c->T = c->Ts; c->Ts = t; }
         c->step += 1;
         if (c->nprobes > 0 && c->step % c->probe_every == 0) append_probes(c);
     }
@@ -451,7 +508,7 @@ void orc_line_rows(const orc_ctx *c, int b, int j, double *A, double *B, double 
             F[i] = 0;
         } else {
             real a, bb, cc, f;
-            regular_row(c, b, i, j, m, (real)tau_d, (real)amp_d, Tm, Tl, Tp, &a, &bb, &cc, &f);
+            regular_row(c, b, i, j, m, (real)tau_d, (real)amp_d, Tm, Tl, Tp, Tm, Tl, Tp, &a, &bb, &cc, &f);
             A[i] = (double)a; B[i] = (double)bb; C[i] = (double)cc; F[i] = (double)f;
         }
     }

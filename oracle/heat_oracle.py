@@ -152,6 +152,7 @@ def _load(variant: str):
         lib.orc_create.argtypes = [C.POINTER(_Desc)]
         lib.orc_destroy.argtypes = [C.c_void_p]
         lib.orc_step.argtypes = [C.c_void_p, C.c_int64]
+        lib.orc_step_picard.argtypes = [C.c_void_p, C.c_int64, C.c_int]
         lib.orc_step_index.restype = C.c_int64
         lib.orc_step_index.argtypes = [C.c_void_p]
         lib.orc_get_field.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
@@ -221,6 +222,10 @@ class Oracle:
 
     def step(self, n: int = 1) -> None:
         self._lib.orc_step(self._h, int(n))
+
+    def step_picard(self, n: int = 1, iters: int = 2) -> None:
+        """n steps of the iterated variant (reading G23); iters = 1 is step()."""
+        self._lib.orc_step_picard(self._h, int(n), int(iters))
 
     def field(self, b: int = 0) -> np.ndarray:
         out = np.empty((self.nz, self.nr), dtype=np.float64)
