@@ -106,12 +106,16 @@ typedef struct {
     int32_t probe_every;             /* record after every probe_every-th step (>= 1 if nprobes) */
     const int32_t *probe_ij;         /* host, nprobes*(i,j)                                      */
     int32_t T_init_is_device;
-    int32_t reserved;
+    int32_t flags;                   /* HEAT_DESC_* bits, 0 = defaults                            */
     double T_lo, T_hi;               /* declared temperature range: every lambda_m, c_Vm must be
                                         strictly positive on it (HEAT_ERANGE otherwise; the
                                         paper's printed graphite c_V row is not, G11).
                                         T_hi <= T_lo disables the check                          */
 } heat_desc;
+
+/* heat_desc.flags: run this context on the general line kernel whatever the grid (needed by
+ * heat_step_picard; also what HEAT_KERNEL=line in the environment does for every context). */
+#define HEAT_DESC_GENERAL_KERNEL 1
 
 /* Bytes of device workspace heat_create needs for this descriptor (0 if it is malformed). */
 size_t heat_workspace_bytes(const heat_desc *d);
@@ -137,6 +141,20 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
 /* Enqueue n solver steps on cuda_stream (asynchronous).  A transient sub-step counts as one
  * step.  The schedule (tau_k, nu_k p_k^2) is derived from integer step counters only. */
 heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream);
+
+/* Variant, not the paper's scheme: "for implicit difference schema with
+ * coefficients depending on the sought-after function (temperature), one needs to make iterations for
+ * evaluation of temperature at each time step", which the paper avoids by its switch-on
+ * sub-stepping.  n solver steps, each as `iters` simple iterations on the coefficients
+ * (reading G23): T^(0) = T; T^(s+1) solves (8)-(20) with every lambda_m, c_Vm and X_m
+ * evaluated at T^(s), the current level T staying in rho c_V (T^ - T)/tau and in Lambda_j[T];
+ * T^ = T^(iters).  iters = 1 is heat_step.  One kernel launch per iteration.
+ *   field_c : device, batch*nz*nr doubles, 16-byte aligned, caller-owned: the second iterate buffer.
+ *             It is scratch between calls (never the current level); its z-boundary lines are set
+ *             up on the first call with this pointer and after heat_set_field / heat_set_line.
+ * Needs a context created with HEAT_DESC_GENERAL_KERNEL (HEAT_EINVAL otherwise).  Schedule, step
+ * counter and probe records advance per solver step, as in heat_step. */
+heat_status heat_step_picard(heat_ctx *c, int64_t n, int32_t iters, void *field_c, void *cuda_stream);
 
 /* Copy the current level of batch member b ([nz][nr], r fastest) to dst.  Asynchronous if
  * dst is a device pointer; synchronises the stream if dst is host memory. */

@@ -19,13 +19,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libheat_b200.so")
 
 HEAT_OK, HEAT_EINVAL, HEAT_ENOMEM, HEAT_ECUDA, HEAT_ERANGE = range(5)
+HEAT_DESC_GENERAL_KERNEL = 1
 STATUS_NAMES = {0: "HEAT_OK", 1: "HEAT_EINVAL", 2: "HEAT_ENOMEM", 3: "HEAT_ECUDA", 4: "HEAT_ERANGE"}
 
 EXPORTS = [
     "heat_workspace_bytes", "heat_stable_dt", "heat_create", "heat_step", "heat_get_field",
     "heat_set_field", "heat_get_line", "heat_set_line", "heat_probe", "heat_schedule", "heat_step_index", "heat_launch_count",
     "heat_kernel_name", "heat_last_error", "heat_destroy", "heat_fp64_peak", "heat_fp64_peak_scratch_bytes",
-    "heat_create_static", "heat_static_workspace_bytes",
+    "heat_create_static", "heat_static_workspace_bytes", "heat_step_picard",
 ]
 
 
@@ -61,7 +62,7 @@ class heat_desc(C.Structure):
         ("transient_k", C.c_double),
         ("nprobes", C.c_int32), ("probe_every", C.c_int32),
         ("probe_ij", C.POINTER(C.c_int32)),
-        ("T_init_is_device", C.c_int32), ("reserved", C.c_int32),
+        ("T_init_is_device", C.c_int32), ("flags", C.c_int32),
         ("T_lo", C.c_double), ("T_hi", C.c_double),
     ]
 
@@ -116,6 +117,8 @@ def lib():
         L.heat_create_static.argtypes = [C.POINTER(heat_desc), vp, vp, vp, C.c_size_t, vp, C.POINTER(vp)]
         L.heat_static_workspace_bytes.restype = C.c_size_t
         L.heat_static_workspace_bytes.argtypes = []
+        L.heat_step_picard.restype = C.c_int
+        L.heat_step_picard.argtypes = [vp, i64, C.c_int32, vp, vp]
         _lib = L
     return _lib
 
@@ -188,6 +191,7 @@ class Desc:
         d.steps_on = int(spec.get("steps_on", 0))
         d.transient_substeps = int(spec.get("transient_substeps", 0))
         d.face_mode = int(spec.get("face_mode", 0))
+        d.flags = HEAT_DESC_GENERAL_KERNEL if spec.get("general_kernel") else 0
         d.transient_k = float(spec.get("transient_k", 7.0))
         d.nprobes = self.probe_ij.shape[0]
         d.probe_every = int(spec.get("probe_every", 1))
@@ -317,6 +321,12 @@ class HeatSim:
     def step(self, n=1):
         """heat_step: enqueue n solver steps (asynchronous)."""
         self._check(self._L.heat_step(self._h, int(n), self._s()))
+
+    def step_picard(self, n=1, iters=2):
+        """heat_step_picard: n solver steps of the iterated variant; needs spec["general_kernel"]."""
+        if getattr(self, "_field_c", None) is None:
+            self._field_c = self._torch.empty_like(self.field_a)
+        self._check(self._L.heat_step_picard(self._h, int(n), int(iters), self._field_c.data_ptr(), self._s()))
 
     def field(self, b=0) -> np.ndarray:
         """heat_get_field to host memory, [nz][nr]."""

@@ -432,6 +432,7 @@ struct heat_ctx {
     CUtensorMap wtm[2]; // [0] = field_a, [1] = field_b; box {16, 32}
     int pdl;                 // band kernel: launch with programmatic stream serialization
     int persist;             // line kernel: heat_step(n >= 2) is one cooperative multi-step launch
+    const void *iter_ready;  // heat_step_picard: the iteration buffer whose Dirichlet z lines are in place
     CUtensorMap btm_ld[2], btm_st[2];
     BParams bp;
     CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
@@ -465,7 +466,7 @@ extern "C" {
 size_t heat_workspace_bytes(const heat_desc *d)
 {
     if (validate(d, nullptr) != HEAT_OK) return 0;
-    const TmaVariant *tv = pick_tma_variant(d->nr);
+    const TmaVariant *tv = (d->flags & HEAT_DESC_GENERAL_KERNEL) ? nullptr : pick_tma_variant(d->nr);
     const Variant *v = tv ? nullptr : pick_variant(d->nr);
     if (!v && !tv) return 0;
     return make_layout(d, v, tv).total;
@@ -526,7 +527,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (!field_a || !field_b || !workspace || field_a == field_b) { set_err(nullptr, "field_a, field_b (distinct) and workspace must be non-NULL device pointers"); return HEAT_EINVAL; }
     if (((uintptr_t)field_a | (uintptr_t)field_b) & 15u) { set_err(nullptr, "field buffers must be 16-byte aligned"); return HEAT_EINVAL; }
     if ((uintptr_t)workspace & 255u) { set_err(nullptr, "workspace must be 256-byte aligned"); return HEAT_EINVAL; }
-    const TmaVariant *tv = pick_tma_variant(d->nr);
+    const TmaVariant *tv = (d->flags & HEAT_DESC_GENERAL_KERNEL) ? nullptr : pick_tma_variant(d->nr);
     const Variant *v = tv ? nullptr : pick_variant(d->nr);
     if (!v && !tv) { set_err(nullptr, "no kernel variant covers nr = %d", d->nr); return HEAT_EINVAL; }
     const Layout L = make_layout(d, v, tv);
@@ -555,8 +556,9 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     std::vector<uint32_t> bdesc;
     std::vector<uint32_t> wdesc;
     const TBandVariant *tbv = nullptr;
-    const WBandVariant *wv = plan_wband(d, &players, &wdesc, &tbv);
-    const BandVariant *bv = wv ? nullptr : plan_band(d, &players, &bdesc);
+    const bool general = (d->flags & HEAT_DESC_GENERAL_KERNEL) != 0;
+    const WBandVariant *wv = general ? nullptr : plan_wband(d, &players, &wdesc, &tbv);
+    const BandVariant *bv = (wv || general) ? nullptr : plan_band(d, &players, &bdesc);
     c->var = v; c->tvar = tv; c->bvar = bv; c->wvar = wv; c->tbvar = tbv; c->lay = L; c->ws = (char *)workspace;
     // measured: 10.4 -> 8.7 us per step on 512 x 512, 36.9 -> 34.7 on 2048 x 2048; with clusters (nr >= 4096)
     // the piecemeal placement of the next step's clusters costs 11 %, so it stays off there
@@ -565,7 +567,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     c->field_a = (double *)field_a;
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
     c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
-    c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0; c->persist = 0;
+    c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0; c->persist = 0; c->iter_ready = nullptr;
 
     // ---- per-node row tables (host), SURVEY 8(a) a4
     const int nr = d->nr, nz = d->nz, N = nr - 1, nrp = L.nrp;
@@ -812,6 +814,10 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occp, (const void *)v->fn_persist, v->tpb, c->smem);
         c->persist = (coop && e == cudaSuccess && (long long)c->grid <= (long long)prop.multiProcessorCount * occp) ? 1 : 0;
         if (const char *ep = getenv("HEAT_PERSIST")) c->persist = c->persist && atoi(ep) != 0;
+        // the iterated variant's kernel (heat_step_picard) is launched in the same shape
+        e = cudaFuncSetAttribute((const void *)v->fn_iter, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(v->smem_fixed + sizeof(DLayer) * (size_t)HEAT_MAX_LAYERS));
+        if (e != cudaSuccess) { set_err(nullptr, "%s (iterated): cannot reserve shared memory: %s", v->name, cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
     }
 
 
@@ -1144,6 +1150,61 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
     return HEAT_OK;
 }
 
+heat_status heat_step_picard(heat_ctx *c, int64_t n, int32_t iters, void *field_c, void *cuda_stream)
+{
+    if (!c || n < 0 || iters < 1) { if (c) set_err(&c->err, "heat_step_picard: bad arguments"); return HEAT_EINVAL; }
+    if (iters == 1) return heat_step(c, n, cuda_stream);
+    if (!c->var || c->tvar || c->bvar || c->wvar) {
+        set_err(&c->err, "heat_step_picard runs on the general line kernel: create the context with HEAT_DESC_GENERAL_KERNEL in heat_desc.flags");
+        return HEAT_EINVAL;
+    }
+    if (!field_c || ((uintptr_t)field_c & 15u) || field_c == (void *)c->cur || field_c == (void *)c->nxt) {
+        set_err(&c->err, "heat_step_picard: field_c must be a third, 16-byte aligned device buffer of batch*nz*nr doubles");
+        return HEAT_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t rec = (size_t)c->batch * (size_t)c->nprobes;
+    const size_t cells = (size_t)c->batch * (size_t)c->nz * (size_t)c->nr;
+    if (c->iter_ready != field_c) {
+        // Dirichlet z lines are never written by a step (G17): the iteration buffer needs them once
+        CUDA_TRY(&c->err, cudaMemcpyAsync(field_c, c->cur, sizeof(double) * cells, cudaMemcpyDeviceToDevice, st));
+        c->iter_ready = field_c;
+    }
+    for (int64_t s = 0; s < n; ++s) {
+        double tau, amp;
+        heat_schedule(c, c->step, &tau, &amp);
+        KParams &k = c->kp;
+        k.Told = c->cur;
+        k.inv_tau = 1.0 / tau;
+        k.amp = amp;
+        double *probe_out = nullptr;
+        if (c->nprobes > 0 && (c->step + 1) % c->probe_every == 0) {
+            if (((size_t)c->rec_enqueued + 1) * rec <= c->probe_cap) {
+                probe_out = c->probe_buf + (size_t)c->rec_enqueued * rec;
+                c->rec_enqueued += 1;
+            } else {
+                c->rec_dropped += 1;
+            }
+        }
+        // iterate it writes c->nxt if (iters - 1 - it) is even, else field_c: the last one lands in c->nxt
+        const double *coef = c->cur;
+        for (int32_t it = 0; it < iters; ++it) {
+            double *out = ((iters - 1 - it) & 1) ? (double *)field_c : c->nxt;
+            k.Tnew = out;
+            k.Tcoef = coef;
+            k.probe_out = (it == iters - 1) ? probe_out : nullptr;
+            if (it == 0) c->var->fn<<<c->grid, c->var->tpb, c->smem, st>>>(k);
+            else c->var->fn_iter<<<c->grid, c->var->tpb, c->smem, st>>>(k);
+            c->launches += 1;
+            coef = out;
+        }
+        std::swap(c->cur, c->nxt);
+        c->step += 1;
+    }
+    CUDA_TRY(&c->err, cudaGetLastError());
+    return HEAT_OK;
+}
+
 heat_status heat_get_field(heat_ctx *c, int32_t b, double *dst, int32_t dst_is_device, void *cuda_stream)
 {
     if (!c || !dst || b < 0 || b >= c->batch) { if (c) set_err(&c->err, "heat_get_field: bad arguments"); return HEAT_EINVAL; }
@@ -1159,6 +1220,7 @@ heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t sr
                            int64_t step_index, void *cuda_stream)
 {
     if (!c || !src || b < 0 || b >= c->batch || step_index < 0) { if (c) set_err(&c->err, "heat_set_field: bad arguments"); return HEAT_EINVAL; }
+    c->iter_ready = nullptr; // an iteration buffer would hold stale z-boundary lines
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t n = (size_t)c->nz * c->nr;
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
@@ -1184,6 +1246,7 @@ heat_status heat_get_line(heat_ctx *c, int32_t b, int32_t j, double *dst, int32_
 heat_status heat_set_line(heat_ctx *c, int32_t b, int32_t j, const double *src, int32_t src_is_device, void *cuda_stream)
 {
     if (!c || !src || b < 0 || b >= c->batch || j < 0 || j >= c->nz) { if (c) set_err(&c->err, "heat_set_line: bad arguments"); return HEAT_EINVAL; }
+    c->iter_ready = nullptr; // an iteration buffer would hold stale z-boundary lines
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t off = ((size_t)b * c->nz + (size_t)j) * (size_t)c->nr;
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;

@@ -150,6 +150,8 @@ struct KParams {
     size_t probe_cap;
     double *probe_base;
     DSched sched;
+    // iterated variant (heat_line_iter_kernel): the field the laws are evaluated at
+    const double *Tcoef;
 };
 
 } // namespace heat

@@ -94,9 +94,13 @@ __device__ __forceinline__ T ldT(const T *ptr)
 }
 
 // One solver step of the lines this CTA owns (grid-stride over groups of LPB lines).
-template <int M, int G, int COH, int TPBMIN = 256>
+// IT = true: the iterated variant (heat_step_picard, reading G23): lambda, c_V and X are
+// evaluated at the field Tcf (the previous iterate of the new level) instead of the current level,
+// which stays where (8) has it: rho c_V (T^ - T)/tau and Lambda_j[T].
+template <int M, int G, int COH, int TPBMIN = 256, bool IT = false>
 __device__ __forceinline__ void line_step(const KParams &p, const double *Told, double *Tnew, double inv_tau_k, double amp_k,
-                                          double *probe_out, double *st, double *xch, const DLayer *lay)
+                                          double *probe_out, double *st, double *xch, const DLayer *lay,
+                                          const double *Tcf = nullptr)
 {
     using Cfg = LineCfg<M, G, TPBMIN>;
     constexpr int TPB = Cfg::TPB;
@@ -142,6 +146,16 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
         Tc[0] = (i0 > 0 && i0 - 1 < nr) ? ldT<COH>(Tl + i0 - 1) : 1.0;
         Tc[M + 1] = (i0 + M < nr) ? ldT<COH>(Tl + i0 + M) : 1.0;
 
+        // ---- the same nodes of the field the laws are evaluated at (iterated variant only)
+        double Sc[IT ? M + 2 : 1];
+        const double *Sl = IT ? Tcf + line : Tl;
+        if (IT) {
+#pragma unroll
+            for (int k = 0; k < M; ++k) Sc[k + 1] = (i0 + k < nr) ? ldT<COH>(Sl + i0 + k) : 1.0;
+            Sc[0] = (i0 > 0 && i0 - 1 < nr) ? ldT<COH>(Sl + i0 - 1) : 1.0;
+            Sc[IT ? M + 1 : 0] = (i0 + M < nr) ? ldT<COH>(Sl + i0 + M) : 1.0;
+        }
+
         const double ezm = __ldg(p.ezm + j), ezp = __ldg(p.ezp + j);
         const double qa = __ldg(p.Q0 + b) * amp_k; // Q0 nu(t_k) p^2(t_k), (2)-(4),(22)
         const double inv_tau = inv_tau_k;
@@ -170,6 +184,12 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
             }
             const double Tdn_k = (k & 1) ? Tdn2.y : Tdn2.x;
             const double Tup_k = (k & 1) ? Tup2.y : Tup2.x;
+            double Sdn_k = Tdn_k, Sup_k = Tup_k;
+            if (IT) {
+                const bool ok = i0 + k < nr;
+                Sdn_k = ok ? ldT<COH>(Sl - nr + i0 + k) : 1.0;
+                Sup_k = ok ? ldT<COH>(Sl + nr + i0 + k) : 1.0;
+            }
             const uint32_t nf = __ldg(info + k);
             const double gak = __ldg(ga + k), gck = __ldg(gc + k);
             const uint32_t kind = nf & 3u;
@@ -180,22 +200,24 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
                 const DLayer &mL = lay[(nf >> 8) & 0xffu];
                 const DLayer &mR = lay[(nf >> 16) & 0xffu];
                 const double T = Tc[k + 1];
+                const double Ts = IT ? Sc[IT ? k + 1 : 0] : T;         // where the laws are evaluated
+                const double TsL = IT ? Sc[IT ? k : 0] : Tc[k], TsR = IT ? Sc[IT ? k + 2 : 0] : Tc[k + 2];
                 const bool reg = (kind == NK_REG);
                 // lambda_{i-1/2,j}, lambda_{i+1/2,j} P:L127; at an interface node
                 // lambda*_m = lambda_m(T_{i*,j}), lambda*_{m+1} = lambda_{m+1}(T_{i*,j}) P:L183
-                const double lamL = law_face(mL.k, T, reg ? Tc[k] : T, fm);
-                const double lamR = law_face(mR.k, T, reg ? Tc[k + 2] : T, fm);
+                const double lamL = law_face(mL.k, Ts, reg ? TsL : Ts, fm);
+                const double lamR = law_face(mR.k, Ts, reg ? TsR : Ts, fm);
                 A = -gak * lamL;
                 C = -gck * lamR;
                 if (reg) {
-                    const double W = law_at(mL.rc, T) * inv_tau;      // rho c_V / tau
-                    const double lamU = law_face(mL.k, T, Tup_k, fm); // lambda_{i,j+1/2}
-                    const double lamD = law_face(mL.k, T, Tdn_k, fm); // lambda_{i,j-1/2}
+                    const double W = law_at(mL.rc, Ts) * inv_tau;      // rho c_V / tau
+                    const double lamU = law_face(mL.k, Ts, Sup_k, fm); // lambda_{i,j+1/2}
+                    const double lamD = law_face(mL.k, Ts, Sdn_k, fm); // lambda_{i,j-1/2}
                     // Lambda_j[T] (11) P:L125
                     double Lj = ezp * (lamU * (Tup_k - T));
                     Lj = fma(-ezm, lamD * (T - Tdn_k), Lj);
                     F = fma(W, T, Lj);
-                    if (mL.heater && qa != 0.0) F = fma(qa, law_at(mL.src, T), F);
+                    if (mL.heater && qa != 0.0) F = fma(qa, law_at(mL.src, Ts), F);
                     B = W - A - C;
                 } else {
                     B = -A - C; // (18) P:L178-181 at the new level (reading G7), scaled by h_i h_{i+1}
@@ -378,6 +400,22 @@ __device__ __forceinline__ void dev_schedule(const DSched &d, long long s, doubl
     } else {
         inv_tau = d.inv_dt; amp = ((s % d.P) < d.S) ? 1.0 : 0.0;
     }
+}
+
+// One iteration of the iterated variant (heat_step_picard): as heat_line_kernel with the laws at p.Tcoef.
+template <int M, int G>
+__global__ void __launch_bounds__(LineCfg<M, G>::TPB) heat_line_iter_kernel(const __grid_constant__ KParams p)
+{
+    using Cfg = LineCfg<M, G>;
+    constexpr int TPB = Cfg::TPB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *st = reinterpret_cast<double *>(smem_raw); // [3][M][TPB]
+    double *xch = st + 3 * M * TPB;                    // [10][NW]
+    DLayer *lay = reinterpret_cast<DLayer *>(xch + 10 * Cfg::NW);
+    for (int q = threadIdx.x; q < p.nlayers * (int)(sizeof(DLayer) / sizeof(int)); q += TPB)
+        reinterpret_cast<int *>(lay)[q] = reinterpret_cast<const int *>(p.layers)[q];
+    __syncthreads();
+    line_step<M, G, 0, 256, true>(p, p.Told, p.Tnew, p.inv_tau, p.amp, p.probe_out, st, xch, lay, p.Tcoef);
 }
 
 // Persistent multi-step version for grids whose CTAs are all resident (cooperative launch): the

@@ -13,7 +13,7 @@ namespace heat {
 typedef void (*kernel_fn)(const KParams);
 struct Variant {
     int M, G, tpb, lpb;
-    kernel_fn fn, fn_persist;
+    kernel_fn fn, fn_persist, fn_iter;
     const char *name;
     size_t smem_fixed; // bytes without the layer table
 };
@@ -25,7 +25,7 @@ extern const int k_nvariants_b;
 #define HEAT_VARIANT(M_, G_)                                                                      \
     {                                                                                             \
         M_, G_, LineCfg<M_, G_>::TPB, LineCfg<M_, G_>::LPB, heat_line_kernel<M_, G_>,             \
-            heat_line_persist_kernel<M_, G_>,                                                     \
+            heat_line_persist_kernel<M_, G_>, heat_line_iter_kernel<M_, G_>,                      \
             "line<M=" #M_ ",G=" #G_ ">", LineCfg<M_, G_>::smem_bytes(0)                           \
     }
 
