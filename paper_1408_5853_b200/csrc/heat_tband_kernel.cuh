@@ -417,14 +417,15 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
         {
             const uint32_t sd = wbase + ((qbase + 0u) % (uint32_t)NS) * (uint32_t)SLOT;
             const uint32_t s1 = wbase + ((qbase + 1u) % (uint32_t)NS) * (uint32_t)SLOT;
-#pragma unroll
+#pragma unroll 1
             for (int g = 0; g < 4; ++g) {
                 double fl[4];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const int q = 2 * g + h;
-                    const double2 td = lds128(sd + co[q]);
-                    const double2 tc = lds128(s1 + co[q]);
+                    const uint32_t oq = A.rowo + ((((uint32_t)q) ^ A.sw) << 4);
+                    const double2 td = lds128(sd + oq);
+                    const double2 tc = lds128(s1 + oq);
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const int k = 2 * q + e;
@@ -434,7 +435,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                         fl[2 * h + e] = wlam<DEGK, true>(c.K, isB ? A.sqB : A.sqA, a_ + d_) * (a_ - d_);
                     }
                 }
-                tmem_st4(tm + tcol_flux(g), fl[0], fl[1], fl[2], fl[3]);
+                tmem_st4(tm + 96u + 8u * (uint32_t)g, fl[0], fl[1], fl[2], fl[3]);
             }
             tmem_wait_st();
         }
