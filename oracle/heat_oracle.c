@@ -23,6 +23,8 @@
  *   G7  (18) second line is at the new level        G8  (22) exponent is negative
  *   G9  source sampled at the start of the step     G14 material belongs to r-segments
  *   G16 Neumann z-line copies its neighbour         G17 Dirichlet z-lines are never solved
+ *   G24 non-rectangular Omega, "N_j" of (9) P:L117 and Fig. 1: a stepped domain -- the lines above z_{j_step}
+ *       end at node i_step (the core reaching the terminal) with zero flux (6) on the two new faces
  *   G23 (variant orc_step_picard only) "iterations at each time step" P:L206 = simple iteration on
  *       the coefficients: laws at the previous iterate, the current level where (8) has it
  *
@@ -93,6 +95,7 @@ typedef struct {
     double transient_k;              /* 7 in the paper */
     int32_t nprobes, probe_every;
     const int32_t *probe_ij;         /* nprobes*(i,j) */
+    int32_t i_step, j_step;          /* stepped domain (G24): lines j > j_step end at node i_step; 0, 0 = rectangle */
 } orc_desc;
 
 typedef struct {
@@ -108,6 +111,7 @@ typedef struct {
     double transient_k;
     int nprobes, probe_every;
     int32_t *probe_ij;
+    int i_step, j_step;
     /* state */
     real *T, *Tn;       /* two time levels, [batch][nz][nr], r fastest */
     real *Ts;           /* iterate of the new level (orc_step_picard only; allocated on first use) */
@@ -220,11 +224,16 @@ static void regular_row(const orc_ctx *c, int b, int i, int j, int m, real tau, 
     *F = rc / tau * T_ij + Lj + X;
 }
 
-/* One line j of batch member b: forward sweep (12),(16),(20), then (17) and back sweep (14). */
+/* One line j of batch member b: forward sweep (12),(16),(20), then (17) and back sweep (14).
+ * N = N_j, the last node of the line (9) P:L117: nr - 1 on a rectangle; on the stepped domain (G24)
+ * the lines above the step end at i_step with the zero-flux condition (6),(15), and the nodes beyond
+ * N_j are not part of Omega: they keep their value. */
 static void line_solve(const orc_ctx *c, int b, int j, real tau, real amp,
                        const real *T, const real *S, real *Tn, real *alpha, real *beta)
 {
-    int nr = c->nr, N = nr - 1;
+    int nr = c->nr;
+    int shortline = (c->j_step > 0 && j > c->j_step);
+    int N = shortline ? c->i_step : nr - 1;
     const real *Tm = T + (size_t)(j - 1) * nr, *Tl = T + (size_t)j * nr, *Tp = T + (size_t)(j + 1) * nr;
     const real *Sm = S + (size_t)(j - 1) * nr, *Sl = S + (size_t)j * nr, *Sp = S + (size_t)(j + 1) * nr;
     real *out = Tn + (size_t)j * nr;
@@ -260,13 +269,24 @@ static void line_solve(const orc_ctx *c, int b, int j, real tau, real amp,
         }
     }
     /* (17) P:L171-174 */
-    if (c->r_out.kind == ORC_BC_NEUMANN0)
+    if (shortline || c->r_out.kind == ORC_BC_NEUMANN0)
         out[N] = beta[N - 1] / (1 - alpha[N - 1]);
     else
         out[N] = (real)c->r_out.value;
+    for (int i = N + 1; i < nr; ++i) out[i] = Tl[i]; /* outside Omega */
     /* (14) P:L150 */
     for (int i = N - 1; i >= 0; --i)
         out[i] = alpha[i] * out[i + 1] + beta[i];
+}
+
+/* Stepped domain (G24): the face z = z_{j_step}, i > i_step carries no flux (6).  First order, like the
+ * z boundaries (G16): the nodes just above it mirror the new values of the nodes below, so that the
+ * explicit flux lambda (T_{i,j+1} - T_{i,j}) / eta through that face is zero in the next step. */
+static void step_face(const orc_ctx *c, real *Tn)
+{
+    if (c->j_step <= 0) return;
+    for (int i = c->i_step + 1; i < c->nr; ++i)
+        Tn[(size_t)(c->j_step + 1) * c->nr + i] = Tn[(size_t)c->j_step * c->nr + i];
 }
 
 /* ------------------------------------------------------------------ life cycle */
@@ -294,6 +314,11 @@ static int validate(const orc_desc *d)
     for (int p = 0; p < d->nprobes; ++p) {
         int i = d->probe_ij[2 * p], j = d->probe_ij[2 * p + 1];
         if (i < 0 || i >= d->nr || j < 0 || j >= d->nz) return 1;
+        if (d->j_step > 0 && j > d->j_step && i > d->i_step) return 1; /* outside Omega */
+    }
+    if (d->j_step != 0 || d->i_step != 0) {
+        if (d->j_step < 1 || d->j_step > d->nz - 3) return 1;
+        if (d->i_step < 2 || d->i_step > d->nr - 2) return 1;
     }
     return 0;
 }
@@ -331,6 +356,7 @@ orc_ctx *orc_create(const orc_desc *d)
     c->transient_substeps = d->transient_substeps; c->face_mode = d->face_mode;
     c->transient_k = d->transient_k;
     c->nprobes = d->nprobes; c->probe_every = d->probe_every;
+    c->i_step = d->i_step; c->j_step = d->j_step;
     c->probe_ij = (int32_t *)dup_mem(d->probe_ij, sizeof(int32_t) * 2 * (size_t)d->nprobes);
     size_t cells = (size_t)d->batch * d->nz * d->nr;
     c->T = (real *)malloc(sizeof(real) * cells);
@@ -357,6 +383,7 @@ orc_ctx *orc_create(const orc_desc *d)
                 for (int i = 0; i < nr; ++i) T[(size_t)(nz - 1) * nr + i] = (real)c->z_hi.value;
         }
     }
+    for (int b = 0; b < c->batch; ++b) step_face(c, c->T + (size_t)b * nz * nr);
     memcpy(c->Tn, c->T, sizeof(real) * cells);
     return c;
 }
@@ -400,6 +427,7 @@ void orc_step(orc_ctx *c, int64_t n)
                 Tn[(size_t)M * nr + i] =
                     (c->z_hi.kind == ORC_BC_DIRICHLET) ? T[(size_t)M * nr + i] : Tn[(size_t)(M - 1) * nr + i];
             }
+            step_face(c, Tn);
         }
         real *t = c->T; c->T = c->Tn; c->Tn = t; /* swap levels */
         c->step += 1;
@@ -441,6 +469,7 @@ void orc_step_picard(orc_ctx *c, int64_t n, int iters)
                     Tn[(size_t)M * nr + i] =
                         (c->z_hi.kind == ORC_BC_DIRICHLET) ? T[(size_t)M * nr + i] : Tn[(size_t)(M - 1) * nr + i];
                 }
+                step_face(c, Tn);
             }
             S = out;                                  /* the next iteration evaluates the laws here */
             out = (out == c->Tn) ? c->Ts : c->Tn;     /* ... and writes into the other buffer */
@@ -469,6 +498,7 @@ void orc_set_field(orc_ctx *c, int b, const double *src, int64_t step_index)
     size_t n = (size_t)c->nz * c->nr;
     real *T = c->T + (size_t)b * n;
     for (size_t k = 0; k < n; ++k) T[k] = (real)src[k];
+    step_face(c, T);
     c->step = step_index;
 }
 
@@ -485,7 +515,9 @@ int64_t orc_probe(const orc_ctx *c, double *dst, int64_t max)
  * interface nodes.  Used by the dense-solve pin: the sweep above never reads these arrays. */
 void orc_line_rows(const orc_ctx *c, int b, int j, double *A, double *B, double *C, double *F)
 {
-    int nr = c->nr, nz = c->nz, N = nr - 1;
+    int nr = c->nr, nz = c->nz;
+    int shortline = (c->j_step > 0 && j > c->j_step);
+    int N = shortline ? c->i_step : nr - 1;
     double tau_d, amp_d;
     orc_schedule(c, c->step, &tau_d, &amp_d);
     const real *T = c->T + (size_t)b * nz * nr;
@@ -493,8 +525,9 @@ void orc_line_rows(const orc_ctx *c, int b, int j, double *A, double *B, double 
     const uint8_t *seg = c->seg_layer + (size_t)b * (nr - 1);
     if (c->r_in.kind == ORC_BC_NEUMANN0) { A[0] = 0; B[0] = 1; C[0] = -1; F[0] = 0; }
     else { A[0] = 0; B[0] = 1; C[0] = 0; F[0] = c->r_in.value; }
-    if (c->r_out.kind == ORC_BC_NEUMANN0) { A[N] = -1; B[N] = 1; C[N] = 0; F[N] = 0; }
+    if (shortline || c->r_out.kind == ORC_BC_NEUMANN0) { A[N] = -1; B[N] = 1; C[N] = 0; F[N] = 0; }
     else { A[N] = 0; B[N] = 1; C[N] = 0; F[N] = c->r_out.value; }
+    for (int i = N + 1; i < nr; ++i) { A[i] = 0; B[i] = 1; C[i] = 0; F[i] = (double)Tl[i]; } /* outside Omega */
     for (int i = 1; i <= N - 1; ++i) {
         int m = seg[i - 1], m1 = seg[i];
         if (m != m1) {

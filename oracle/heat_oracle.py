@@ -66,6 +66,7 @@ class _Desc(C.Structure):
         ("transient_k", C.c_double),
         ("nprobes", C.c_int32), ("probe_every", C.c_int32),
         ("probe_ij", C.POINTER(C.c_int32)),
+        ("i_step", C.c_int32), ("j_step", C.c_int32),
     ]
 
 
@@ -138,6 +139,7 @@ class _Marshalled:
         d.nprobes = self.probe_ij.shape[0]
         d.probe_every = int(spec.get("probe_every", 1))
         d.probe_ij = self.probe_ij.ctypes.data_as(C.POINTER(C.c_int32))
+        d.i_step, d.j_step = int(spec.get("i_step", 0)), int(spec.get("j_step", 0))
         self.desc = d
         self.nr, self.nz, self.batch = nr, nz, batch
 
