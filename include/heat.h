@@ -111,6 +111,14 @@ typedef struct {
                                         strictly positive on it (HEAT_ERANGE otherwise; the
                                         paper's printed graphite c_V row is not, G11).
                                         T_hi <= T_lo disables the check                          */
+    int32_t i_step, j_step;          /* stepped domain (reading G24 of "N_j" in
+                                        the grid (9) P:L117 and of Fig. 1): the lines j > j_step end at
+                                        node i_step (the core reaching the terminal) with zero flux (6) on
+                                        the two new faces; the nodes i > i_step of those lines are not part
+                                        of Omega: they are never solved, the line j_step + 1 of them mirrors
+                                        line j_step (no flux through the step face), whatever T_init holds
+                                        there.  0, 0 = rectangle.  2 <= i_step <= nr-2, 1 <= j_step <= nz-3;
+                                        runs on the general line kernel                           */
 } heat_desc;
 
 /* heat_desc.flags: run this context on the general line kernel whatever the grid (needed by

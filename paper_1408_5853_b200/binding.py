@@ -64,6 +64,7 @@ class heat_desc(C.Structure):
         ("probe_ij", C.POINTER(C.c_int32)),
         ("T_init_is_device", C.c_int32), ("flags", C.c_int32),
         ("T_lo", C.c_double), ("T_hi", C.c_double),
+        ("i_step", C.c_int32), ("j_step", C.c_int32),
     ]
 
 
@@ -192,6 +193,7 @@ class Desc:
         d.transient_substeps = int(spec.get("transient_substeps", 0))
         d.face_mode = int(spec.get("face_mode", 0))
         d.flags = HEAT_DESC_GENERAL_KERNEL if spec.get("general_kernel") else 0
+        d.i_step, d.j_step = int(spec.get("i_step", 0)), int(spec.get("j_step", 0))
         d.transient_k = float(spec.get("transient_k", 7.0))
         d.nprobes = self.probe_ij.shape[0]
         d.probe_every = int(spec.get("probe_every", 1))

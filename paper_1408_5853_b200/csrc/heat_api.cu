@@ -327,7 +327,7 @@ constexpr int k_range_samples = 1025;
 // ---------------------------------------------------------------- workspace layout
 struct Layout {
     int nrp;
-    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, off_wdesc, off_ampsub, total;
+    size_t off_ga, off_gc, off_info, off_ezm, off_ezp, off_layers, off_q0, off_probes, off_cdesc, off_bdesc, off_players, off_wdesc, off_ampsub, off_ga2, off_gc2, off_info2, total;
 };
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -350,6 +350,12 @@ Layout make_layout(const heat_desc *d, const Variant *v, const TmaVariant *tv)
     L.off_players = o; o = align_up(o + sizeof(PLayer) * (size_t)HEAT_MAX_LAYERS, 256);
     L.off_wdesc = o;  o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * (size_t)(d->nr / 16 + 1), 256);
     L.off_ampsub = o; o = align_up(o + sizeof(double) * (size_t)(d->transient_substeps + 1), 256);
+    L.off_ga2 = L.off_gc2 = L.off_info2 = 0;
+    if (d->j_step > 0) { // stepped domain: the row tables of the lines above the step
+        L.off_ga2 = o;   o = align_up(o + sizeof(double) * (size_t)d->batch * L.nrp, 256);
+        L.off_gc2 = o;   o = align_up(o + sizeof(double) * (size_t)d->batch * L.nrp, 256);
+        L.off_info2 = o; o = align_up(o + sizeof(uint32_t) * (size_t)d->batch * L.nrp, 256);
+    }
     L.total = o;
     return L;
 }
@@ -395,6 +401,14 @@ heat_status validate(const heat_desc *d, std::string *err)
         for (int q = 0; q < d->nprobes; ++q) {
             const int i = d->probe_ij[2 * q], j = d->probe_ij[2 * q + 1];
             if (i < 0 || i >= d->nr || j < 0 || j >= d->nz) { set_err(err, "probe %d = (%d,%d) outside the grid", q, i, j); return HEAT_EINVAL; }
+            if (d->j_step > 0 && j > d->j_step && i > d->i_step) { set_err(err, "probe %d = (%d,%d) lies outside the stepped domain", q, i, j); return HEAT_EINVAL; }
+        }
+    }
+    // stepped domain (reading G24)
+    if (d->i_step != 0 || d->j_step != 0) {
+        if (d->j_step < 1 || d->j_step > d->nz - 3 || d->i_step < 2 || d->i_step > d->nr - 2) {
+            set_err(err, "stepped domain: need 1 <= j_step <= nz-3 and 2 <= i_step <= nr-2 (got i_step = %d, j_step = %d)", d->i_step, d->j_step);
+            return HEAT_EINVAL;
         }
     }
     // strictly positive laws on the declared range (the paper's own graphite c_V row fails, G11)
@@ -433,6 +447,7 @@ struct heat_ctx {
     int pdl;                 // band kernel: launch with programmatic stream serialization
     int persist;             // line kernel: heat_step(n >= 2) is one cooperative multi-step launch
     const void *iter_ready;  // heat_step_picard: the iteration buffer whose Dirichlet z lines are in place
+    int i_step, j_step;      // stepped domain (reading G24); 0, 0 = rectangle
     CUtensorMap btm_ld[2], btm_st[2];
     BParams bp;
     CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
@@ -452,6 +467,15 @@ struct heat_ctx {
     KParams kp;
 };
 
+// Stepped domain: the nodes above the step face (line j_step + 1, i > i_step) mirror line j_step of the
+// same level, so that the explicit flux through the face is zero (reading G24, as a Neumann z line G16).
+static cudaError_t mirror_step_face(const heat_ctx *c, double *level, int b, cudaStream_t st)
+{
+    if (c->j_step <= 0) return cudaSuccess;
+    double *line = level + ((size_t)b * c->nz + (size_t)c->j_step) * (size_t)c->nr + (size_t)c->i_step + 1;
+    return cudaMemcpyAsync(line + c->nr, line, sizeof(double) * (size_t)(c->nr - 1 - c->i_step), cudaMemcpyDeviceToDevice, st);
+}
+
 #define CUDA_TRY(ctx_err, call)                                                                   \
     do {                                                                                          \
         cudaError_t e_ = (call);                                                                  \
@@ -466,7 +490,7 @@ extern "C" {
 size_t heat_workspace_bytes(const heat_desc *d)
 {
     if (validate(d, nullptr) != HEAT_OK) return 0;
-    const TmaVariant *tv = (d->flags & HEAT_DESC_GENERAL_KERNEL) ? nullptr : pick_tma_variant(d->nr);
+    const TmaVariant *tv = ((d->flags & HEAT_DESC_GENERAL_KERNEL) || d->j_step > 0) ? nullptr : pick_tma_variant(d->nr);
     const Variant *v = tv ? nullptr : pick_variant(d->nr);
     if (!v && !tv) return 0;
     return make_layout(d, v, tv).total;
@@ -527,7 +551,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     if (!field_a || !field_b || !workspace || field_a == field_b) { set_err(nullptr, "field_a, field_b (distinct) and workspace must be non-NULL device pointers"); return HEAT_EINVAL; }
     if (((uintptr_t)field_a | (uintptr_t)field_b) & 15u) { set_err(nullptr, "field buffers must be 16-byte aligned"); return HEAT_EINVAL; }
     if ((uintptr_t)workspace & 255u) { set_err(nullptr, "workspace must be 256-byte aligned"); return HEAT_EINVAL; }
-    const TmaVariant *tv = (d->flags & HEAT_DESC_GENERAL_KERNEL) ? nullptr : pick_tma_variant(d->nr);
+    const TmaVariant *tv = ((d->flags & HEAT_DESC_GENERAL_KERNEL) || d->j_step > 0) ? nullptr : pick_tma_variant(d->nr);
     const Variant *v = tv ? nullptr : pick_variant(d->nr);
     if (!v && !tv) { set_err(nullptr, "no kernel variant covers nr = %d", d->nr); return HEAT_EINVAL; }
     const Layout L = make_layout(d, v, tv);
@@ -556,7 +580,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     std::vector<uint32_t> bdesc;
     std::vector<uint32_t> wdesc;
     const TBandVariant *tbv = nullptr;
-    const bool general = (d->flags & HEAT_DESC_GENERAL_KERNEL) != 0;
+    const bool general = (d->flags & HEAT_DESC_GENERAL_KERNEL) != 0 || d->j_step > 0;
     const WBandVariant *wv = general ? nullptr : plan_wband(d, &players, &wdesc, &tbv);
     const BandVariant *bv = (wv || general) ? nullptr : plan_band(d, &players, &bdesc);
     c->var = v; c->tvar = tv; c->bvar = bv; c->wvar = wv; c->tbvar = tbv; c->lay = L; c->ws = (char *)workspace;
@@ -601,6 +625,19 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
                 gcb[i] = (double)h_i;
                 ib[i] = NK_IFACE | (m << 8) | (m1 << 16);
             }
+        }
+    }
+    // stepped domain (reading G24): the lines j > j_step end at N_j = i_step with the row (15), the
+    // nodes beyond keep their value
+    std::vector<double> ga2, gc2;
+    std::vector<uint32_t> info2;
+    if (d->j_step > 0) {
+        ga2 = ga; gc2 = gc; info2 = info;
+        for (int b = 0; b < d->batch; ++b) {
+            const size_t o = (size_t)b * nrp;
+            info2[o + (size_t)d->i_step] = NK_FIXED | (3u << 2);
+            ga2[o + (size_t)d->i_step] = -1.0; gc2[o + (size_t)d->i_step] = 0.0;
+            for (int i = d->i_step + 1; i < nr; ++i) { info2[o + (size_t)i] = NK_KEEP; ga2[o + (size_t)i] = 0.0; gc2[o + (size_t)i] = 0.0; }
         }
     }
     std::vector<double> ezm((size_t)nz, 0.0), ezp((size_t)nz, 0.0);
@@ -692,6 +729,11 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     UP(L.off_ga, ga, double);
     UP(L.off_gc, gc, double);
     UP(L.off_info, info, uint32_t);
+    if (d->j_step > 0) {
+        UP(L.off_ga2, ga2, double);
+        UP(L.off_gc2, gc2, double);
+        UP(L.off_info2, info2, uint32_t);
+    }
     UP(L.off_ezm, ezm, double);
     UP(L.off_ezp, ezp, double);
     UP(L.off_layers, lay, DLayer);
@@ -729,6 +771,11 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         }
         e = cudaStreamSynchronize(st); // `one` is pageable host memory reused across copies
         if (e != cudaSuccess) { set_err(nullptr, "stream sync failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
+    }
+    c->i_step = d->i_step; c->j_step = d->j_step;
+    for (int b = 0; b < d->batch && d->j_step > 0; ++b) {
+        e = mirror_step_face(c, c->cur, b, st);
+        if (e != cudaSuccess) { set_err(nullptr, "step-face copy failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
     }
     e = cudaMemcpyAsync(c->nxt, c->cur, sizeof(double) * cells, cudaMemcpyDeviceToDevice, st);
     if (e != cudaSuccess) { set_err(nullptr, "level copy failed: %s", cudaGetErrorString(e)); return fail(HEAT_ECUDA); }
@@ -1015,7 +1062,11 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     k.probes = (const ProbeSrc *)(c->ws + L.off_probes);
     k.fixF[0] = (d->r_in.kind == HEAT_BC_DIRICHLET) ? d->r_in.value : 0.0;
     k.fixF[1] = (d->r_out.kind == HEAT_BC_DIRICHLET) ? d->r_out.value : 0.0;
-    k.fixF[2] = 0.0; k.fixF[3] = 0.0;
+    k.fixF[2] = 0.0; k.fixF[3] = 0.0; // [3]: the (15) row at the end of a line above the step
+    k.i_step = d->i_step; k.j_step = d->j_step;
+    k.ga2 = d->j_step > 0 ? (const double *)(c->ws + L.off_ga2) : nullptr;
+    k.gc2 = d->j_step > 0 ? (const double *)(c->ws + L.off_gc2) : nullptr;
+    k.info2 = d->j_step > 0 ? (const uint32_t *)(c->ws + L.off_info2) : nullptr;
     k.nr = nr; k.nz = nz; k.batch = d->batch; k.nrp = nrp; k.nlayers = d->nlayers; k.nprobes = d->nprobes;
     k.face_mode = d->face_mode;
     k.z_lo_neumann = (d->z_lo.kind == HEAT_BC_NEUMANN0);
@@ -1226,6 +1277,7 @@ heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t sr
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     // both levels: the Dirichlet z lines are never written by a step (G17)
     CUDA_TRY(&c->err, cudaMemcpyAsync(c->cur + (size_t)b * n, src, sizeof(double) * n, kind, st));
+    CUDA_TRY(&c->err, mirror_step_face(c, c->cur, b, st));
     CUDA_TRY(&c->err, cudaMemcpyAsync(c->nxt + (size_t)b * n, c->cur + (size_t)b * n, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
     if (!src_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
     c->step = step_index;
@@ -1252,6 +1304,10 @@ heat_status heat_set_line(heat_ctx *c, int32_t b, int32_t j, const double *src, 
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     CUDA_TRY(&c->err, cudaMemcpyAsync(c->cur + off, src, sizeof(double) * (size_t)c->nr, kind, st));
     CUDA_TRY(&c->err, cudaMemcpyAsync(c->nxt + off, c->cur + off, sizeof(double) * (size_t)c->nr, cudaMemcpyDeviceToDevice, st));
+    if (c->j_step > 0 && (j == c->j_step || j == c->j_step + 1)) {
+        CUDA_TRY(&c->err, mirror_step_face(c, c->cur, b, st));
+        CUDA_TRY(&c->err, mirror_step_face(c, c->nxt, b, st));
+    }
     if (!src_is_device) CUDA_TRY(&c->err, cudaStreamSynchronize(st));
     return HEAT_OK;
 }

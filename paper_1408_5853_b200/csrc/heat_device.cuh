@@ -43,7 +43,7 @@ struct DLayer {
 
 // node kinds in the per-node info word: bits 0-1 kind, bits 2-3 fixed-row slot,
 // bits 8-15 layer of the segment left of the node, bits 16-23 layer right of it
-enum : uint32_t { NK_REG = 0, NK_IFACE = 1, NK_FIXED = 2 };
+enum : uint32_t { NK_REG = 0, NK_IFACE = 1, NK_FIXED = 2, NK_KEEP = 3 }; // NK_KEEP: outside Omega (stepped domain), x = T
 
 __device__ __forceinline__ double rcp_nr(double x)
 {
@@ -152,6 +152,11 @@ struct KParams {
     DSched sched;
     // iterated variant (heat_line_iter_kernel): the field the laws are evaluated at
     const double *Tcoef;
+    // stepped domain (reading G24): the lines j > j_step use the second set of row tables, in which node
+    // i_step is the (15) boundary row and the nodes beyond it are NK_KEEP; j_step = 0: rectangle
+    const double *ga2, *gc2;
+    const uint32_t *info2;
+    int i_step, j_step;
 };
 
 } // namespace heat

@@ -113,7 +113,8 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
     const int wig = t >> 5;    // warp within the group
     const int gw0 = (grp * G) >> 5; // first warp of the group (MULTI only)
     const int nr = p.nr, nz = p.nz;
-    const bool vec_ok = ((nr & 1) == 0);
+    const bool stepped = (p.j_step > 0);
+    const bool vec_ok = ((nr & 1) == 0) && !stepped; // the step may fall between the two nodes of a pair
     const int interior = nz - 2;
 
     for (int base = blockIdx.x * Cfg::LPB; base < p.total_lines; base += gridDim.x * Cfg::LPB) {
@@ -126,9 +127,10 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
         const double *Tl = Told + line;
         const double *Tm = Tl - nr;
         const double *Tp = Tl + nr;
-        const double *ga = p.ga + (size_t)b * p.nrp + i0;
-        const double *gc = p.gc + (size_t)b * p.nrp + i0;
-        const uint32_t *info = p.info + (size_t)b * p.nrp + i0;
+        const bool upper = stepped && j > p.j_step; // a line above the step: N_j = i_step
+        const double *ga = (upper ? p.ga2 : p.ga) + (size_t)b * p.nrp + i0;
+        const double *gc = (upper ? p.gc2 : p.gc) + (size_t)b * p.nrp + i0;
+        const uint32_t *info = (upper ? p.info2 : p.info) + (size_t)b * p.nrp + i0;
 
         // ---- load line j (current level) for the thread's nodes, plus the halo
         double Tc[M + 2];
@@ -196,6 +198,8 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
             double A, B, C, F;
             if (kind == NK_FIXED) {
                 A = gak; B = 1.0; C = gck; F = p.fixF[(nf >> 2) & 3u];
+            } else if (kind == NK_KEEP) {
+                A = 0.0; B = 1.0; C = 0.0; F = Tc[k + 1]; // outside Omega: the node keeps its value
             } else {
                 const DLayer &mL = lay[(nf >> 8) & 0xffu];
                 const DLayer &mR = lay[(nf >> 16) & 0xffu];
@@ -345,7 +349,11 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
 #pragma unroll
                 for (int k = 0; k < M; ++k) {
                     if (i0 + k < nr) {
-                        out[i0 + k] = x[k];
+                        // stepped domain: the nodes above the step face mirror line j_step (no flux through
+                        // the face, as a Neumann z line G16); line j_step + 1 itself leaves them alone
+                        const bool beyond = stepped && (i0 + k > p.i_step);
+                        if (!(beyond && j == p.j_step + 1)) out[i0 + k] = x[k];
+                        if (beyond && j == p.j_step) out[i0 + k + nr] = x[k];
                         if (lo) out[i0 + k - nr] = x[k];
                         if (hi) out[i0 + k + nr] = x[k];
                     }

@@ -320,6 +320,7 @@ PAPER_RHO = (8.92, 2.0, 2.0, 2.5)
 # This is OUR substitution, not the paper's number; heat_create rejects the printed row.
 PAPER_GRAPHITE_A3_SUBSTITUTE = -8.199e-9
 PAPER_RADII_CM = (0.12, 0.125, 0.13, 0.1301)   # r_0, r_1, r_2, r_max
+PAPER_Z0_CM = 4.0                              # end of the layered part (reading G10 of the garbled P:L241)
 PAPER_ZMAX_CM = 5.0                            # P:L300 (z_0 = 4 cm, reading G10, is not needed on a rectangle)
 PAPER_I0_A, PAPER_CHI0 = 0.363, 1.8            # I_0 P:L278; chi(T) = 1.8 / sqrt(T) Ohm cm, (25) P:L274
 PAPER_T0, PAPER_TCRIT = 4.2, 42.2
@@ -367,7 +368,7 @@ def paper_radial_nodes(nr=631):
     return r, [n_core, n_core + n1, n_core + n1 + n2]
 
 
-def paper_device(M=201, nr=631, tau=1e-5, printed_graphite=False):
+def paper_device(M=201, nr=631, tau=1e-5, printed_graphite=False, stepped=False):
     """The workload of the paper's section 5: radii 0.12 / 0.125 / 0.13 / 0.1301 cm,
     z_max = 5 cm, POLY laws of Tables 2-3, source chi(T) I_0^2 / S_2^2 in the conducting layer with
     I_0 = 363 mA, zero flux everywhere except T = 4.2 K at z_max (6), T_0 = 4.2 K, tau = 1e-5 s,
@@ -390,4 +391,10 @@ def paper_device(M=201, nr=631, tau=1e-5, printed_graphite=False):
     s["probes"] = [(nr - 1, 0), (nr - 1, M // 2), (0, 0)]           # Fig. 7 probe, mid surface, axis
     s["probe_every"] = 1
     s["name"] = f"paper device {nr}x{M}"
+    if stepped:
+        # Fig. 1 with reading G10 (z_0 = 4 cm): the layers 1-3 end at z_0, the copper core (r <= r_0, the
+        # first interface node) goes on to the terminal at z_max; reading G24 of the non-rectangular Omega
+        s["i_step"] = int(ifaces[0])
+        s["j_step"] = int(round(PAPER_Z0_CM / PAPER_ZMAX_CM * (M - 1)))
+        s["name"] += " stepped"
     return s

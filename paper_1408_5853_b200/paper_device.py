@@ -29,6 +29,8 @@ def main():
     ap.add_argument("--periods", type=int, default=400, help="source periods of the long run (400 = 10 s)")
     ap.add_argument("--M", type=int, default=201)
     ap.add_argument("--timing", action="store_true", help="also time the six grids of Table 4")
+    ap.add_argument("--stepped", action="store_true",
+                    help="the geometry of Fig. 1: layers 1-3 end at z_0 = 4 cm, the core goes on to the terminal (row f2, reading G24)")
     ap.add_argument("--out", default="gpurun_out/paper_device")
     args = ap.parse_args()
 
@@ -56,7 +58,7 @@ def main():
             print(lines[-1], flush=True)
             sim.close()
 
-    s = I.paper_device(args.M)
+    s = I.paper_device(args.M, stepped=args.stepped)
     P, nsub, S = int(s["steps_per_period"]), int(s["transient_substeps"]), int(s["steps_on"])
     per = P - 1 + nsub                       # solver steps per period
     on_steps = nsub + S - 1                  # solver steps until the source switches off
@@ -64,7 +66,7 @@ def main():
     nr, nz = sim.nr, sim.nz
     z = np.asarray(s["z"])
     work = z <= 4.0 + 1e-12                  # working surface z in [0, z_0], P:L314 (z_0 = 4 cm, reading G10)
-    lines.append(f"long run: {nr} x {nz}, tau = {s['dt']:.1e} s, {per} solver steps per period, kernel {sim.kernel_name}")
+    lines.append(f"long run: {s['name']}, {nr} x {nz}, tau = {s['dt']:.1e} s, {per} solver steps per period, kernel {sim.kernel_name}")
     t0 = time.time()
     rows = []
     for n in range(args.periods):

@@ -115,3 +115,16 @@ def test_design_sweep_host_logic():
         nodes = np.flatnonzero(np.diff(s["seg_layer"][b].astype(int))) + 1
         assert nodes[0] == 420 and nodes[2] == 620 and nodes[1] == 620 - th[b]
     assert binding.heat_workspace_bytes(s) > 0
+
+
+def test_paper_device_stepped_geometry():
+    """Fig. 1 with reading G10 / G24: the step sits on the first interface node (r_0 = 0.12 cm) and on z_0 = 4 cm."""
+    from oracle.heat_oracle import Oracle
+    s = I.paper_device(M=201, stepped=True)
+    assert s["r"][s["i_step"]] == pytest.approx(0.12) and s["z"][s["j_step"]] == pytest.approx(4.0)
+    assert s["seg_layer"][0][s["i_step"] - 1] == 0 and s["seg_layer"][0][s["i_step"]] == 1
+    o = Oracle(s)
+    o.step(120)
+    F = o.field()
+    assert np.all(F[s["j_step"] + 2:-1, s["i_step"] + 1:] == 4.2)      # outside Omega
+    assert F[: s["j_step"] + 1].max() > 6.0
