@@ -182,6 +182,27 @@ heat_status heat_set_field(heat_ctx *c, int32_t b, const double *src, int32_t sr
 heat_status heat_get_line(heat_ctx *c, int32_t b, int32_t j, double *dst, int32_t dst_is_device, void *cuda_stream);
 heat_status heat_set_line(heat_ctx *c, int32_t b, int32_t j, const double *src, int32_t src_is_device, void *cuda_stream);
 
+/* z-slab multi-GPU run with direct peer stores instead of heat_get_line / heat_set_line:
+ * tell this context where a neighbour slab keeps its two field levels.  From then on every heat_step
+ * also stores this slab's first interior line (side 0: the neighbour below) or last interior line
+ * (side 1: the neighbour above) of the NEW level into the neighbour's halo line -- its last line
+ * (side 0) or its line 0 (side 1) -- of the neighbour's NEXT level: the level buffer with the same
+ * position (a / b) as this context's next level.  The store is issued by the step kernel itself (a TMA
+ * store in the tband kernel, plain stores in the line kernel), so over NVLink the exchange overlaps the
+ * rest of the step; no other call moves halo data.
+ *   peer_field_a, peer_field_b : the field_a, field_b the neighbour passed to ITS heat_create, as
+ *                                addresses valid on this device (same GPU, or peer-mapped: P2P access
+ *                                enabled / cudaIpcOpenMemHandle); NULL, NULL switches the side off
+ *   peer_nz                    : the neighbour's nz (its halo lines included); nr and batch are this context's
+ * Contract: all slabs start from the same level (a freshly created context, or the same number of steps)
+ * and advance in lock step -- one heat_step(1) each, then a synchronisation between the ranks (the
+ * neighbour reads the stored line in its next step) -- so the level written is never the one a
+ * neighbour's running step reads.  The side that faces a neighbour must be a Dirichlet z line.
+ * Available for contexts on the tband and the line kernel (HEAT_EINVAL otherwise); multi-step
+ * persistent launches are off while a peer is set, and heat_step_picard with iters > 1 is refused (its
+ * iterates would need an exchange per iteration). */
+heat_status heat_set_halo_peer(heat_ctx *c, int32_t side, void *peer_field_a, void *peer_field_b, int32_t peer_nz);
+
 /* Drain the probe trace: synchronise cuda_stream, copy up to max doubles (whole records of
  * batch*nprobes doubles, order [record][batch][probe]) to dst_host, and rewind the device
  * buffer.  *n_written = doubles copied; *n_dropped (optional) = records lost to overflow. */

@@ -26,7 +26,7 @@ EXPORTS = [
     "heat_workspace_bytes", "heat_stable_dt", "heat_create", "heat_step", "heat_get_field",
     "heat_set_field", "heat_get_line", "heat_set_line", "heat_probe", "heat_schedule", "heat_step_index", "heat_launch_count",
     "heat_kernel_name", "heat_last_error", "heat_destroy", "heat_fp64_peak", "heat_fp64_peak_scratch_bytes",
-    "heat_create_static", "heat_static_workspace_bytes", "heat_step_picard",
+    "heat_create_static", "heat_static_workspace_bytes", "heat_step_picard", "heat_set_halo_peer",
 ]
 
 
@@ -118,6 +118,8 @@ def lib():
         L.heat_create_static.argtypes = [C.POINTER(heat_desc), vp, vp, vp, C.c_size_t, vp, C.POINTER(vp)]
         L.heat_static_workspace_bytes.restype = C.c_size_t
         L.heat_static_workspace_bytes.argtypes = []
+        L.heat_set_halo_peer.restype = C.c_int
+        L.heat_set_halo_peer.argtypes = [vp, C.c_int32, vp, vp, C.c_int32]
         L.heat_step_picard.restype = C.c_int
         L.heat_step_picard.argtypes = [vp, i64, C.c_int32, vp, vp]
         _lib = L
@@ -368,6 +370,17 @@ class HeatSim:
         else:
             v = np.ascontiguousarray(np.asarray(values, dtype=np.float64).reshape(self.nr))
             self._check(self._L.heat_set_line(self._h, int(b), int(j), C.c_void_p(v.ctypes.data), 0, self._s()))
+
+    def set_halo_peer(self, side, peer=None):
+        """heat_set_halo_peer: `peer` is the neighbour slab's HeatSim in this process (side 0: the slab below,
+        1: above), a tuple (field_a_ptr, field_b_ptr, nz) of peer-mapped addresses, or None to switch it off."""
+        if peer is None:
+            a, b, pnz = None, None, 0
+        elif isinstance(peer, tuple):
+            a, b, pnz = peer
+        else:
+            a, b, pnz = peer.field_a.data_ptr(), peer.field_b.data_ptr(), peer.nz
+        self._check(self._L.heat_set_halo_peer(self._h, int(side), a, b, int(pnz)))
 
     def probes(self, max_records=None):
         """heat_probe: drain the trace, shape [records, batch, nprobes]; also returns drops."""

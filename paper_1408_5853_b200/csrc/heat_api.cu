@@ -448,6 +448,9 @@ struct heat_ctx {
     int persist;             // line kernel: heat_step(n >= 2) is one cooperative multi-step launch
     const void *iter_ready;  // heat_step_picard: the iteration buffer whose Dirichlet z lines are in place
     int i_step, j_step;      // stepped domain (reading G24); 0, 0 = rectangle
+    double *peer[2][2];      // heat_set_halo_peer: [side][level] the neighbour slab's field_a / field_b, or NULL
+    int peer_nz[2];
+    CUtensorMap wtm_peer[2][2]; // tband: tensor maps over them
     CUtensorMap btm_ld[2], btm_st[2];
     BParams bp;
     CUtensorMap tm_ld[2], tm_st[2]; // [0] = field_a, [1] = field_b
@@ -474,6 +477,32 @@ static cudaError_t mirror_step_face(const heat_ctx *c, double *level, int b, cud
     if (c->j_step <= 0) return cudaSuccess;
     double *line = level + ((size_t)b * c->nz + (size_t)c->j_step) * (size_t)c->nr + (size_t)c->i_step + 1;
     return cudaMemcpyAsync(line + c->nr, line, sizeof(double) * (size_t)(c->nr - 1 - c->i_step), cudaMemcpyDeviceToDevice, st);
+}
+
+// z-slab run with direct peer stores: point this launch at the neighbours' NEXT level (the buffer with
+// the index of this context's next level: all slabs advance in lock step from the same starting level)
+static void set_peer_params(heat_ctx *c, KParams &k, bool on)
+{
+    const int lvl = (c->nxt == c->field_a) ? 0 : 1;
+    WParams &wp = c->wp;
+    k.peer_lo = k.peer_hi = nullptr; k.peer_lo_stride = k.peer_hi_stride = 0;
+    wp.peer_lo_row = wp.peer_hi_row = -1;
+    if (!on) return;
+    const long long nr = c->nr;
+    if (c->peer[0][lvl]) { // lower neighbour: its last line is its upper halo line
+        k.peer_lo = c->peer[0][lvl] + (long long)(c->peer_nz[0] - 1) * nr;
+        k.peer_lo_stride = (long long)c->peer_nz[0] * nr;
+        wp.tm_peer_lo = c->wtm_peer[0][lvl];
+        wp.peer_lo_row = (int)((long long)(c->peer_nz[0] - 1) * nr / 16);
+        wp.peer_lo_rpm = (int)((long long)c->peer_nz[0] * nr / 16);
+    }
+    if (c->peer[1][lvl]) { // upper neighbour: its line 0 is its lower halo line
+        k.peer_hi = c->peer[1][lvl];
+        k.peer_hi_stride = (long long)c->peer_nz[1] * nr;
+        wp.tm_peer_hi = c->wtm_peer[1][lvl];
+        wp.peer_hi_row = 0;
+        wp.peer_hi_rpm = (int)((long long)c->peer_nz[1] * nr / 16);
+    }
 }
 
 #define CUDA_TRY(ctx_err, call)                                                                   \
@@ -592,6 +621,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
     c->cur = (double *)field_a; c->nxt = (double *)field_b;
     c->probe_buf = (double *)probe_buf; c->probe_cap = probe_cap;
     c->rec_enqueued = c->rec_dropped = 0; c->step = 0; c->launches = 0; c->persist = 0; c->iter_ready = nullptr;
+    c->peer[0][0] = c->peer[0][1] = c->peer[1][0] = c->peer[1][1] = nullptr; c->peer_nz[0] = c->peer_nz[1] = 0;
 
     // ---- per-node row tables (host), SURVEY 8(a) a4
     const int nr = d->nr, nz = d->nz, N = nr - 1, nrp = L.nrp;
@@ -1031,6 +1061,7 @@ heat_status heat_create(const heat_desc *d, void *field_a, void *field_b, void *
         }
         WParams &wp = c->wp;
         memset(&wp, 0, sizeof wp);
+        wp.peer_lo_row = wp.peer_hi_row = -1;
         wp.wdesc = (const uint32_t *)(c->ws + L.off_wdesc);
         wp.players = (const PLayer *)(c->ws + L.off_players);
         wp.ezm = (const double *)(c->ws + L.off_ezm);
@@ -1089,7 +1120,8 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
     if (!c || n < 0) return HEAT_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t rec = (size_t)c->batch * (size_t)c->nprobes;
-    if (c->persist && !c->bvar && !c->tvar && !c->wvar && n >= 2) {
+    const bool peers = c->peer[0][0] != nullptr || c->peer[1][0] != nullptr; // the ranks synchronise after every step
+    if (c->persist && !c->bvar && !c->tvar && !c->wvar && n >= 2 && !peers) {
         // one cooperative launch per chunk: schedule, level swap and probe slots run on the device
         int64_t left = n;
         while (left > 0) {
@@ -1130,6 +1162,7 @@ heat_status heat_step(heat_ctx *c, int64_t n, void *cuda_stream)
                 c->rec_dropped += 1;
             }
         }
+        set_peer_params(c, k, true);
         if (c->wvar) {
             const int q = (c->cur == c->field_a) ? 0 : 1;
             WParams &wp = c->wp;
@@ -1209,6 +1242,12 @@ heat_status heat_step_picard(heat_ctx *c, int64_t n, int32_t iters, void *field_
         set_err(&c->err, "heat_step_picard runs on the general line kernel: create the context with HEAT_DESC_GENERAL_KERNEL in heat_desc.flags");
         return HEAT_EINVAL;
     }
+    if (c->peer[0][0] != nullptr || c->peer[1][0] != nullptr) {
+        // every iterate reads the neighbours' previous iterate on the halo lines: a slab run would need an
+        // exchange per iteration, which heat_set_halo_peer does not do
+        set_err(&c->err, "heat_step_picard with iters > 1 is not available on a slab with halo peers");
+        return HEAT_EINVAL;
+    }
     if (!field_c || ((uintptr_t)field_c & 15u) || field_c == (void *)c->cur || field_c == (void *)c->nxt) {
         set_err(&c->err, "heat_step_picard: field_c must be a third, 16-byte aligned device buffer of batch*nz*nr doubles");
         return HEAT_EINVAL;
@@ -1253,6 +1292,46 @@ heat_status heat_step_picard(heat_ctx *c, int64_t n, int32_t iters, void *field_
         c->step += 1;
     }
     CUDA_TRY(&c->err, cudaGetLastError());
+    return HEAT_OK;
+}
+
+heat_status heat_set_halo_peer(heat_ctx *c, int32_t side, void *peer_field_a, void *peer_field_b, int32_t peer_nz)
+{
+    if (!c || side < 0 || side > 1) { if (c) set_err(&c->err, "heat_set_halo_peer: side is 0 (lower neighbour) or 1 (upper)"); return HEAT_EINVAL; }
+    if (!peer_field_a && !peer_field_b) { c->peer[side][0] = c->peer[side][1] = nullptr; c->peer_nz[side] = 0; return HEAT_OK; }
+    if (!peer_field_a || !peer_field_b || peer_nz < 3 || (((uintptr_t)peer_field_a | (uintptr_t)peer_field_b) & 15u)) {
+        set_err(&c->err, "heat_set_halo_peer: need both level buffers of the neighbour (16-byte aligned) and its nz >= 3");
+        return HEAT_EINVAL;
+    }
+    if (!c->tbvar && (c->tvar || c->bvar || c->wvar)) { // heat_step's order of precedence: tband, wband, band, tma, line
+        set_err(&c->err, "heat_set_halo_peer: peer stores are built into the tband and the line kernel (this context runs %s)", heat_kernel_name(c));
+        return HEAT_EINVAL;
+    }
+    if ((side == 0 && c->z_lo.kind != HEAT_BC_DIRICHLET) || (side == 1 && c->z_hi.kind != HEAT_BC_DIRICHLET)) {
+        set_err(&c->err, "heat_set_halo_peer: the side that faces a neighbour slab must be a Dirichlet z line (the halo line)");
+        return HEAT_EINVAL;
+    }
+    double *lev[2] = {(double *)peer_field_a, (double *)peer_field_b};
+    if (c->tbvar) {
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || !sym || qres != cudaDriverEntryPointSuccess) { set_err(&c->err, "cuTensorMapEncodeTiled is unavailable (%s)", cudaGetErrorString(e)); return HEAT_ECUDA; }
+        const cuuint64_t gdim[2] = {16, (cuuint64_t)c->batch * (cuuint64_t)peer_nz * (cuuint64_t)c->nr / 16};
+        const cuuint64_t gstr[1] = {128};
+        const cuuint32_t estr[2] = {1, 1};
+        const cuuint32_t box[2] = {16, 32};
+        for (int q = 0; q < 2; ++q) {
+            CUresult r = ((encode_fn)sym)(&c->wtm_peer[side][q], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, lev[q], gdim, gstr, box, estr,
+                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) { set_err(&c->err, "cuTensorMapEncodeTiled on the neighbour's buffer failed (%d)", (int)r); return HEAT_ECUDA; }
+        }
+    }
+    c->peer[side][0] = lev[0]; c->peer[side][1] = lev[1]; c->peer_nz[side] = peer_nz;
     return HEAT_OK;
 }
 

@@ -157,6 +157,10 @@ struct KParams {
     const double *ga2, *gc2;
     const uint32_t *info2;
     int i_step, j_step;
+    // z-slab run with direct peer stores (heat_set_halo_peer): where the first / last interior line of
+    // the new level goes in the lower / upper neighbour slab's next level (batch member 0; nullptr: none)
+    double *peer_lo, *peer_hi;
+    long long peer_lo_stride, peer_hi_stride; // doubles per batch member there
 };
 
 } // namespace heat

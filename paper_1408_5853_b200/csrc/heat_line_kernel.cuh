@@ -359,6 +359,16 @@ __device__ __forceinline__ void line_step(const KParams &p, const double *Told, 
                     }
                 }
             }
+            // ---- z-slab run: the neighbour slabs' halo lines get this slab's edge lines (peer stores)
+            if ((j == 1 && p.peer_lo != nullptr) || (j == nz - 2 && p.peer_hi != nullptr)) {
+#pragma unroll
+                for (int k = 0; k < M; ++k) {
+                    if (i0 + k < nr) {
+                        if (j == 1 && p.peer_lo != nullptr) p.peer_lo[(long long)b * p.peer_lo_stride + i0 + k] = x[k];
+                        if (j == nz - 2 && p.peer_hi != nullptr) p.peer_hi[(long long)b * p.peer_hi_stride + i0 + k] = x[k];
+                    }
+                }
+            }
             // ---- probes: T of the new level at (i_p, j_p)
             if (probe_out != nullptr) {
                 for (int q = 0; q < p.nprobes; ++q) {

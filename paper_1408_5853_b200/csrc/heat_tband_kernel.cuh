@@ -596,8 +596,13 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             if (lane == 0) {
                 const int Rg = (b * nz + j) * rpl + wig * 32;
                 tma_store_2d(&p.tm_st, 0, Rg, sc);
-                if (j == 1 && p.z_lo_neumann) tma_store_2d(&p.tm_st, 0, Rg - rpl, sc);
-                if (j == nz - 2 && p.z_hi_neumann) tma_store_2d(&p.tm_st, 0, Rg + rpl, sc);
+                if (j == 1 || j == nz - 2) { // the edge lines of the grid
+                    if (j == 1 && p.z_lo_neumann) tma_store_2d(&p.tm_st, 0, Rg - rpl, sc);
+                    if (j == nz - 2 && p.z_hi_neumann) tma_store_2d(&p.tm_st, 0, Rg + rpl, sc);
+                    // z-slab run: the neighbour slabs' halo lines get this slab's edge lines over NVLink / peer memory
+                    if (j == 1 && p.peer_lo_row >= 0) tma_store_2d(&p.tm_peer_lo, 0, p.peer_lo_row + b * p.peer_lo_rpm + wig * 32, sc);
+                    if (j == nz - 2 && p.peer_hi_row >= 0) tma_store_2d(&p.tm_peer_hi, 0, p.peer_hi_row + b * p.peer_hi_rpm + wig * 32, sc);
+                }
                 tma_commit();
             }
 

@@ -44,6 +44,11 @@ struct WParams {
     int rpl;  // tensor rows (16 doubles) per line = threads per line
     int BL;   // lines per band
     int bands_per_member, total_bands;
+    // z-slab run with direct peer stores (heat_set_halo_peer): the first / last interior line of the new
+    // level is also stored into the halo line of the lower / upper neighbour slab's NEXT level
+    CUtensorMap tm_peer_lo, tm_peer_hi;
+    int peer_lo_row, peer_hi_row;   // tensor row of batch member 0's halo line there, < 0: no such neighbour
+    int peer_lo_rpm, peer_hi_rpm;   // tensor rows per batch member there
 };
 
 // WL = warps per line (nr = 512 WL), NW = warps per CTA.  A line wider than a CTA spans a cluster

@@ -20,6 +20,13 @@ GPU, the oracle in the CPU test); the transport is torch.distributed send / recv
 gloo in the CPU test) or a direct copy when both slabs live in one process.
 Probes stay with the rank that owns their line (`local_probes`).  No scaling curve has been measured:
 this sandbox has one GPU.
+
+Peer-store mode (`peer_plan`, `connect_peers_in_one_process`, `step_peer_slabs_in_one_process`): instead of
+get_line / send / recv / set_line, `heat_set_halo_peer` gives every slab the address of its neighbours' field
+levels and the step kernel itself stores its edge lines into their halo lines (TMA store / plain stores
+over NVLink peer memory), so the exchange costs no extra kernel or copy and overlaps the step.  Between
+processes the addresses come from cudaIpcOpenMemHandle and the per-step synchronisation is a barrier;
+that wiring needs several GPUs and is not in this file.
 """
 from __future__ import annotations
 
@@ -148,6 +155,34 @@ def step_slabs_in_one_process(steppers, nz: int, n: int = 1):
         for peer, jr, lines in moved:
             for b in range(batch):
                 steppers[peer].set_line(b, jr, lines[b])
+
+
+def peer_plan(rank: int, world: int):
+    """Peer-store mode (heat_set_halo_peer): [(side, neighbour rank)] -- side 0 is the slab below, 1 the slab above."""
+    plan = []
+    if rank > 0:
+        plan.append((0, rank - 1))
+    if rank < world - 1:
+        plan.append((1, rank + 1))
+    return plan
+
+
+def connect_peers_in_one_process(steppers):
+    """Every slab's step kernel stores its edge lines straight into its neighbours' halo lines (all slabs
+    in this process: the same GPU, or GPUs with peer access enabled).  After this, a step of the run is
+    `for st in steppers: st.step(1)` plus a synchronisation; no get_line / set_line."""
+    world = len(steppers)
+    for r, st in enumerate(steppers):
+        for side, peer in peer_plan(r, world):
+            st.set_halo_peer(side, steppers[peer])
+
+
+def step_peer_slabs_in_one_process(steppers, n: int = 1):
+    """n steps in peer-store mode.  In one process the launches are ordered by the stream: step k of
+    every slab is enqueued before step k + 1 of any (between processes this is a barrier per step)."""
+    for _ in range(n):
+        for st in steppers:
+            st.step(1)
 
 
 def gather_field(fields, nz: int):

@@ -693,3 +693,66 @@ def test_zslab_run_equals_the_single_gpu_run_bitwise(bd, nr, nz, world):
     one.close()
     for q in slabs:
         q.close()
+
+
+@pytest.mark.parametrize("nr,nz,world,batch", [(512, 40, 2, 1), (1024, 23, 3, 1), (2048, 20, 2, 1), (96, 30, 2, 1), (77, 31, 3, 2)])
+def test_zslab_peer_stores_equal_the_single_gpu_run_bitwise(bd, nr, nz, world, batch):
+    """heat_set_halo_peer: the step kernel itself stores a slab's edge lines into its neighbours' halo lines
+    (TMA store in the tband kernel, plain stores in the line kernel); no get_line / set_line.  On ONE GPU the
+    "peer" buffers are the other contexts' fields and the launches are ordered by the stream.  The gathered
+    field must be bitwise the single-context field."""
+    from paper_1408_5853_b200 import zslab as Z
+    if nr == 77:
+        s0 = I.random_spec(9, nr=nr, nz=nz, nlayers=3, batch=batch, bcs=(I.NEUMANN0, I.NEUMANN0, I.dirichlet(4.2), I.dirichlet(78.0)))
+        s0["general_kernel"] = True
+        s = with_dt(bd, s0)
+    else:
+        s = with_dt(bd, I.config(2, nr=nr, nz=nz))
+    one = bd.HeatSim(s)
+    slabs = [bd.HeatSim(Z.slab_spec(s, r, world)) for r in range(world)]
+    assert all(q.kernel_name == one.kernel_name for q in slabs)
+    Z.connect_peers_in_one_process(slabs)
+    for n in (1, 60, 31):
+        one.step(1)
+        one.step(n - 1)          # the single run may use its persistent multi-step launch
+        Z.step_peer_slabs_in_one_process(slabs, n)
+        got = Z.gather_field([q.fields() for q in slabs], nz)
+        assert np.array_equal(got, one.fields())
+    if nr == 77:   # iterations would need an exchange per iteration: refused on a slab with peers
+        with pytest.raises(bd.HeatError) as e:
+            slabs[0].step_picard(1, 3)
+        assert "halo peers" in str(e.value)
+    # a peer switched off stops the exchange: the runs part
+    slabs[0].set_halo_peer(1, None)
+    one.step(5)
+    Z.step_peer_slabs_in_one_process(slabs, 5)
+    assert not np.array_equal(Z.gather_field([q.fields() for q in slabs], nz), one.fields())
+    one.close()
+    for q in slabs:
+        q.close()
+
+
+def test_halo_peer_argument_checks(bd):
+    s = with_dt(bd, I.config(2, nr=512, nz=24))
+    a, b = bd.HeatSim(s), bd.HeatSim(s)
+    for side, peer, msg in ((2, b, "side"), (0, (a.field_a.data_ptr(), None, 24), "both level buffers"), (0, (8, 16, 2), "nz >= 3")):
+        with pytest.raises(bd.HeatError) as e:
+            a.set_halo_peer(side, peer)
+        assert e.value.status == bd.HEAT_EINVAL and msg in str(e.value)
+    n0 = dict(s)
+    n0["z_lo"] = I.NEUMANN0
+    c = bd.HeatSim(n0)
+    with pytest.raises(bd.HeatError) as e:
+        c.set_halo_peer(0, b)
+    assert "Dirichlet" in str(e.value)
+    os.environ["HEAT_KERNEL"] = "tma"
+    try:
+        d = bd.HeatSim(s)
+        with pytest.raises(bd.HeatError) as e:
+            d.set_halo_peer(0, b)
+        assert "tband and the line kernel" in str(e.value)
+        d.close()
+    finally:
+        del os.environ["HEAT_KERNEL"]
+    for q in (a, b, c):
+        q.close()

@@ -116,3 +116,16 @@ def test_two_ranks_over_gloo_equal_the_single_run():
     ref = Oracle(s)
     ref.step(17)
     assert np.array_equal(Z.gather_field(fields, s["nz"]), ref.fields())
+
+
+def test_peer_plan_mirrors_the_exchange_plan():
+    """Peer-store mode: a slab stores into exactly the neighbours it would send to, on the side that faces them."""
+    for world in (1, 2, 3, 5):
+        for rank in range(world):
+            plan = Z.peer_plan(rank, world)
+            ex = Z.exchange_plan(40, rank, world)
+            assert [p for _, p in plan] == [p for p, _, _ in ex]
+            for side, peer in plan:
+                assert peer == rank - 1 if side == 0 else peer == rank + 1
+                # the neighbour lists this rank on its opposite side
+                assert (1 - side, rank) in Z.peer_plan(peer, world)
