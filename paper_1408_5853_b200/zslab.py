@@ -25,8 +25,8 @@ Peer-store mode (`peer_plan`, `connect_peers_in_one_process`, `step_peer_slabs_i
 get_line / send / recv / set_line, `heat_set_halo_peer` gives every slab the address of its neighbours' field
 levels and the step kernel itself stores its edge lines into their halo lines (TMA store / plain stores
 over NVLink peer memory), so the exchange costs no extra kernel or copy and overlaps the step.  Between
-processes the addresses come from cudaIpcOpenMemHandle and the per-step synchronisation is a barrier;
-that wiring needs several GPUs and is not in this file.
+processes (`PeerSlabRank`) the addresses come from CUDA IPC handles and the per-step synchronisation is a
+barrier; tested with two processes sharing the one GPU of this sandbox.
 """
 from __future__ import annotations
 
@@ -183,6 +183,57 @@ def step_peer_slabs_in_one_process(steppers, n: int = 1):
     for _ in range(n):
         for st in steppers:
             st.step(1)
+
+
+def export_level(t):
+    """What another process needs to map a device tensor (one field level): torch's CUDA IPC descriptor of
+    its storage plus the tensor's offset inside it.  The exporting process must keep `t` alive."""
+    return tuple(t.untyped_storage()._share_cuda_()) + (int(t.storage_offset()) * t.element_size(),)
+
+
+def import_level(desc):
+    """(storage to keep alive, device address) of a level exported by another process: cudaIpcOpenMemHandle
+    through torch (peer access between the two GPUs is enabled by the open)."""
+    import torch
+    st = torch.UntypedStorage._new_shared_cuda(*desc[:-1])
+    return st, int(st.data_ptr()) + int(desc[-1])
+
+
+class PeerSlabRank:
+    """One rank of a z-slab run in peer-store mode, one process per GPU.  The addresses of the neighbours'
+    field levels are exchanged once (CUDA IPC handles through `dist.all_gather_object`, any backend); a
+    step is heat_step(1) on every rank, whose kernel stores the edge lines into the neighbours' halo lines,
+    then a stream synchronisation and a barrier: nobody starts step k + 1 before every store of step k
+    has landed.  No halo data passes through the host or through a collective."""
+
+    def __init__(self, sim, rank: int, world: int, dist):
+        self.sim, self.rank, self.world, self.dist = sim, rank, world, dist
+        mine = (export_level(sim.field_a), export_level(sim.field_b), int(sim.nz))
+        everyone = [None] * world
+        dist.all_gather_object(everyone, mine)
+        self._mapped = []
+        for side, peer in peer_plan(rank, world):
+            da, db, pnz = everyone[peer]
+            sa, pa = import_level(da)
+            sb, pb = import_level(db)
+            self._mapped += [sa, sb]
+            sim.set_halo_peer(side, (pa, pb, pnz))
+        dist.barrier()
+
+    def step(self, n: int = 1):
+        for _ in range(n):
+            self.sim.step(1)
+            self.sim.synchronize()
+            self.dist.barrier()
+
+    def close(self):
+        """Stop storing into the neighbours and unmap them (call on every rank before the fields are freed)."""
+        self.sim.synchronize()
+        self.dist.barrier()
+        for side, _ in peer_plan(self.rank, self.world):
+            self.sim.set_halo_peer(side, None)
+        self._mapped = []
+        self.dist.barrier()
 
 
 def gather_field(fields, nz: int):

@@ -756,3 +756,42 @@ def test_halo_peer_argument_checks(bd):
         del os.environ["HEAT_KERNEL"]
     for q in (a, b, c):
         q.close()
+
+
+def _peer_worker(rank, world, port, nr, nz, nsteps, out):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    import torch
+    import torch.distributed as dist
+    from paper_1408_5853_b200 import binding, zslab as Z
+    torch.cuda.set_device(0)                      # one GPU in this sandbox: both ranks share it
+    dist.init_process_group("gloo")
+    s0 = I.config(2, nr=nr, nz=nz)
+    s = I.with_dt(s0, binding.heat_stable_dt(s0))
+    sim = binding.HeatSim(Z.slab_spec(s, rank, world))
+    rk = Z.PeerSlabRank(sim, rank, world, dist)
+    rk.step(nsteps)
+    out[rank] = (sim.kernel_name, sim.fields())
+    rk.close()
+    sim.close()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("nr,nz,world", [(512, 40, 2), (96, 30, 2)])
+def test_zslab_peer_stores_across_processes(bd, nr, nz, world):
+    """PeerSlabRank: one process per rank (here sharing the one GPU), the neighbours' field levels mapped
+    through CUDA IPC, a barrier per step (host-side: no kernel waits on another).  Gathered field == the
+    single run, bitwise."""
+    import torch.multiprocessing as mp
+    from paper_1408_5853_b200 import zslab as Z
+    nsteps = 45
+    port = 33000 + os.getpid() % 2000
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_peer_worker, args=(world, port, nr, nz, nsteps, out), nprocs=world, join=True)
+        res = [out[r] for r in range(world)]
+    s = with_dt(bd, I.config(2, nr=nr, nz=nz))
+    one = bd.HeatSim(s)
+    one.step(nsteps)
+    assert all(name == one.kernel_name for name, _ in res)
+    assert np.array_equal(Z.gather_field([f for _, f in res], nz), one.fields())
+    one.close()
