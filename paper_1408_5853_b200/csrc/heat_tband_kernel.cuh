@@ -104,7 +104,8 @@ struct TSweepArgs {
     uint32_t tm;             // tensor-memory address of the warp's strip (column 0)
     uint32_t rowo, sw;       // byte offset of the thread's tensor row in a slot, its swizzle phase
     uint32_t layA, layB;     // shared addresses of the WLayer before / from the interface row on
-    double hl, hr;           // r neighbours of the chunk at line j
+    double hl;               // left r neighbour of the chunk at line j
+    uint32_t hra;            // shared address of a 16-byte pair whose first double is the right r neighbour
     double fi0, g0, ezp, ezm;
     double gl0;              // geometric factor of the face i0 - 1/2 (0 in the chunk that starts with a Neumann r_in row)
     double fie15;            // capacity / rhs factor of row 15 (0 in the chunk that ends with a Neumann r_out row)
@@ -169,8 +170,10 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &
     const uint32_t o0 = A.rowo + (((q0) ^ A.sw) << 4), o1 = A.rowo + (((q0 + 1u) ^ A.sw) << 4);
     const uint32_t o2 = A.rowo + (((q0 + 2u) & 7u) ^ A.sw) * 16u;
     const double2 t1 = lds128(A.sc + o1);
-    double2 t2 = lds128(A.sc + o2); // rows 4g+4, 4g+5 (the next group's first pair); beyond the chunk: hr
-    if (g == 3) t2 = make_double2(A.hr, A.hr);
+    // rows 4g+4, 4g+5 (the next group's first pair); beyond the chunk: the right neighbour's pair (one select
+    // on the address instead of four on the data); the line's last thread has none and mirrors its own node
+    double2 t2 = lds128((g == 3) ? A.hra : A.sc + o2);
+    if (GEN && g == 3 && A.last) t2.x = t1.y;
     const double2 u0 = lds128(A.su + o0), u1 = lds128(A.su + o1);
     const double fig = A.fi0 + (double)(4 * g);
     const bool lastg = (g == 3);
@@ -461,19 +464,14 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             wait_seq((uint32_t)(L + 2));
 
             // ---- the two r neighbours of the thread's 16 nodes at line j
-            double hl, hr;
-            {
-                const double2 v0 = lds128(sc + co[0]);
-                const double2 v7 = lds128(sc + co[7]);
-                hl = v0.x; hr = v7.y;
-            }
+            double hl;
             if (lane > 0) hl = lds64(sc + hlo);
             else if (has_l) hl = lds64(halo_a + qs * 32u + 8u);
-            if (lane < 31) hr = lds64(sc + hro);
-            else if (has_r) hr = lds64(halo_a + qs * 32u + 16u);
+            else hl = lds64(sc + co[0]);
+            A.hra = (lane < 31) ? sc + hro : has_r ? halo_a + qs * 32u + 16u : sc + co[7];
 
             // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 16 rows
-            A.sc = sc; A.su = su; A.hl = hl; A.hr = hr; A.fi0 = fi0; A.ezp = ezp; A.ezm = ezm;
+            A.sc = sc; A.su = su; A.hl = hl; A.fi0 = fi0; A.ezp = ezp; A.ezm = ezm;
             const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, c, genmask, spmask) : tsweep16<DEGK, false>(A, c, genmask, spmask);
             tmem_wait_st();
             // the slot of line j - 1 has been stored (its TMA store was issued a whole sweep ago): refill it
