@@ -106,7 +106,8 @@ struct TSweepArgs {
     uint32_t layA, layB;     // shared addresses of the WLayer before / from the interface row on
     double hl;               // left r neighbour of the chunk at line j
     uint32_t hra;            // shared address of a 16-byte pair whose first double is the right r neighbour
-    double fi0, g0, ezp, ezm;
+    int i0v;                 // index of the thread's first node (made opaque per line, see the kernel)
+    double g0, ezp, ezm;
     double gl0;              // geometric factor of the face i0 - 1/2 (0 in the chunk that starts with a Neumann r_in row)
     double fie15;            // capacity / rhs factor of row 15 (0 in the chunk that ends with a Neumann r_out row)
     double qsA, qsB;         // source term X (2)-(4),(22) of the two layers
@@ -160,7 +161,10 @@ __device__ __forceinline__ TRowCoef<DEGK> trow_coef(uint32_t a)
 //              coefficients are read row by row from the shared table.  Still no branch per row.
 // The caller picks the body per warp and group (warp-uniform), so the common case runs the plain body
 // and the instruction cache holds four rows of each kind instead of sixteen.
-template <int DEGK, bool SQ, bool GEN>
+// LASTG: 0 / 1 = this is not / is the group with row 15 (known at compile time: the one-line-per-CTA kernel
+// peels the last group, so that the other three carry no selects for it), 2 = decided by g at run time (the
+// smaller CTAs, where several CTAs per SM sit at different places of the code and its size matters more)
+template <int DEGK, bool SQ, bool GEN, int LASTG>
 __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &c, SweepState &st, TSweepOut &o,
                                        double2 &tl, double lamA_if, double lamB_if, uint32_t spmask)
 {
@@ -172,11 +176,11 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &
     const double2 t1 = lds128(A.sc + o1);
     // rows 4g+4, 4g+5 (the next group's first pair); beyond the chunk: the right neighbour's pair (one select
     // on the address instead of four on the data); the line's last thread has none and mirrors its own node
-    double2 t2 = lds128((g == 3) ? A.hra : A.sc + o2);
-    if (GEN && g == 3 && A.last) t2.x = t1.y;
+    const bool lastg = (LASTG == 2) ? (g == 3) : (LASTG == 1);
+    double2 t2 = lds128(lastg ? A.hra : A.sc + o2);
+    if (GEN && lastg && A.last) t2.x = t1.y;
     const double2 u0 = lds128(A.su + o0), u1 = lds128(A.su + o1);
-    const double fig = A.fi0 + (double)(4 * g);
-    const bool lastg = (g == 3);
+    const int ig = A.i0v + 4 * g; // node index of the group's first row; i -> double on the conversion unit, not the FP64 pipe
     const uint32_t ksw = (GEN && A.ks >= 0) ? (uint32_t)A.ks : 99u;
     tmem_wait_ld(fraw);
     double fD[4], cf[12], fu[4];
@@ -188,7 +192,7 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &
         const double Tr = (r == 0) ? tl.y : (r == 1) ? t1.x : (r == 2) ? t1.y : t2.x;
         const double Tu = (r == 0) ? u0.x : (r == 1) ? u0.y : (r == 2) ? u1.x : u1.y;
         const uint32_t k = 4u * (uint32_t)g + (uint32_t)r;
-        const double fi = fig + (double)r;
+        const double fi = (double)(ig + r);
         double cfR, w, f, alk;
         // GEN: only the rows that are special in SOME lane of the warp (warp-uniform bit of spmask) take
         // the general code; the thread that holds the interface row switches its coefficients to layer B
@@ -233,9 +237,11 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &
         }
         cf[3 * r] = alk; cf[3 * r + 1] = st.be; cf[3 * r + 2] = st.gm;
         // x_0 = P x_{k+1} + Q + S u (rows 0 .. 14)
-        const double Qn = fma(o.P, st.be, o.Q), Sn = fma(o.P, st.gm, o.S), Pn = o.P * alk;
-        if (r < 3) { o.Q = Qn; o.S = Sn; o.P = Pn; }
-        else { o.Q = lastg ? o.Q : Qn; o.S = lastg ? o.S : Sn; o.P = lastg ? o.P : Pn; }
+        if (r < 3 || LASTG != 1) {
+            const double Qn = fma(o.P, st.be, o.Q), Sn = fma(o.P, st.gm, o.S), Pn = o.P * alk;
+            if (r < 3 || LASTG == 0) { o.Q = Qn; o.S = Sn; o.P = Pn; }
+            else { o.Q = lastg ? o.Q : Qn; o.S = lastg ? o.S : Sn; o.P = lastg ? o.P : Pn; }
+        }
     }
     tl = t2;
     const uint32_t tc = A.tm + 24u * (uint32_t)g;
@@ -249,7 +255,7 @@ __device__ __forceinline__ void tgroup(const TSweepArgs &A, int g, WCoef<DEGK> &
 // Level 1 for one thread: the sixteen rows in four groups of four (a rolled loop); (alpha, beta,
 // gamma) and the new face fluxes of a group go to tensor memory, the prefix products for the reduced
 // row are carried along.  genmask: bit g set = group g of this warp needs the general body.
-template <int DEGK, bool SQ>
+template <int DEGK, bool SQ, bool PEEL>
 __device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, WCoef<DEGK> &c, uint32_t genmask, uint32_t spmask)
 {
     SweepState st;
@@ -272,10 +278,20 @@ __device__ __forceinline__ TSweepOut tsweep16(const TSweepArgs &A, WCoef<DEGK> &
     }
     double2 tl = lds128(A.sc + A.rowo + (A.sw << 4));
     st.cfL = wlam<DEGK, SQ>(c.K, c.sq, A.hl + tl.x) * A.gl0; // face i0 - 1/2
+    if (PEEL) {
 #pragma unroll 1
-    for (int g = 0; g < 4; ++g) {
-        if (!((genmask >> g) & 1u)) tgroup<DEGK, SQ, false>(A, g, c, st, o, tl, lamA_if, lamB_if, 0u);
-        else tgroup<DEGK, SQ, true>(A, g, c, st, o, tl, lamA_if, lamB_if, spmask);
+        for (int g = 0; g < 3; ++g) {
+            if (!((genmask >> g) & 1u)) tgroup<DEGK, SQ, false, 0>(A, g, c, st, o, tl, lamA_if, lamB_if, 0u);
+            else tgroup<DEGK, SQ, true, 0>(A, g, c, st, o, tl, lamA_if, lamB_if, spmask);
+        }
+        if (!((genmask >> 3) & 1u)) tgroup<DEGK, SQ, false, 1>(A, 3, c, st, o, tl, lamA_if, lamB_if, 0u);
+        else tgroup<DEGK, SQ, true, 1>(A, 3, c, st, o, tl, lamA_if, lamB_if, spmask);
+    } else {
+#pragma unroll 1
+        for (int g = 0; g < 4; ++g) {
+            if (!((genmask >> g) & 1u)) tgroup<DEGK, SQ, false, 2>(A, g, c, st, o, tl, lamA_if, lamB_if, 0u);
+            else tgroup<DEGK, SQ, true, 2>(A, g, c, st, o, tl, lamA_if, lamB_if, spmask);
+        }
     }
     return o;
 }
@@ -361,7 +377,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
 
     const int nz = p.nz, rpl = p.rpl, BL = p.BL, bpm = p.bands_per_member;
     const double g0 = p.g0;
-    double fi0 = (double)i0;
+    int i0v = i0;
     uint32_t qbase = 0;  // load sequence number of line offset -1 of this band
     uint32_t lcount = 0; // lines done (phase of the exchange barriers)
 
@@ -460,7 +476,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             const uint32_t su = wbase + qu * (uint32_t)SLOT; // line j+1 (up)
             const int j = j0 + L;
             const double ezm = __ldg(p.ezm + j), ezp = __ldg(p.ezp + j);
-            asm volatile("" : "+d"(fi0)); // keep the per-row geometry out of registers across lines
+            asm volatile("" : "+r"(i0v)); // keep the per-row geometry out of registers across lines
             wait_seq((uint32_t)(L + 2));
 
             // ---- the two r neighbours of the thread's 16 nodes at line j
@@ -471,8 +487,9 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             A.hra = (lane < 31) ? sc + hro : has_r ? halo_a + qs * 32u + 16u : sc + co[7];
 
             // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 16 rows
-            A.sc = sc; A.su = su; A.hl = hl; A.fi0 = fi0; A.ezp = ezp; A.ezm = ezm;
-            const TSweepOut o = anysq ? tsweep16<DEGK, true>(A, c, genmask, spmask) : tsweep16<DEGK, false>(A, c, genmask, spmask);
+            A.sc = sc; A.su = su; A.hl = hl; A.i0v = i0v; A.ezp = ezp; A.ezm = ezm;
+            constexpr bool PEEL = (NW == 16);
+            const TSweepOut o = anysq ? tsweep16<DEGK, true, PEEL>(A, c, genmask, spmask) : tsweep16<DEGK, false, PEEL>(A, c, genmask, spmask);
             tmem_wait_st();
             // the slot of line j - 1 has been stored (its TMA store was issued a whole sweep ago): refill it
             if (lane == 0 && L >= 1 && L + NS <= nl + 1) { tma_wait_read0(); issue_load((uint32_t)(L + NS)); }
