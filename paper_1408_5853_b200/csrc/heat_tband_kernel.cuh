@@ -480,10 +480,8 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             wait_seq((uint32_t)(L + 2));
 
             // ---- the two r neighbours of the thread's 16 nodes at line j
-            double hl;
-            if (lane > 0) hl = lds64(sc + hlo);
-            else if (has_l) hl = lds64(halo_a + qs * 32u + 8u);
-            else hl = lds64(sc + co[0]);
+            // (one load through a selected address: three branches would diverge between lane 0 and the rest)
+            const double hl = lds64((lane > 0) ? sc + hlo : has_l ? halo_a + qs * 32u + 8u : sc + co[0]);
             A.hra = (lane < 31) ? sc + hro : has_r ? halo_a + qs * 32u + 16u : sc + co[7];
 
             // ---- level 1: assemble (13)/(15)/(18) and sweep (12) the thread's 16 rows
