@@ -91,6 +91,28 @@ __device__ __forceinline__ void tmem_wait_ld3(TRaw8 &a, TRaw8 &b, TRaw8 &c)
                    "+r"(c.r[0]), "+r"(c.r[1]), "+r"(c.r[2]), "+r"(c.r[3]), "+r"(c.r[4]), "+r"(c.r[5]), "+r"(c.r[6]), "+r"(c.r[7])
                  :: "memory");
 }
+struct TRaw16 {
+    uint32_t r[16];
+};
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, TRaw16 &v)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(v.r[0]), "=r"(v.r[1]), "=r"(v.r[2]), "=r"(v.r[3]), "=r"(v.r[4]), "=r"(v.r[5]), "=r"(v.r[6]), "=r"(v.r[7]),
+                   "=r"(v.r[8]), "=r"(v.r[9]), "=r"(v.r[10]), "=r"(v.r[11]), "=r"(v.r[12]), "=r"(v.r[13]), "=r"(v.r[14]), "=r"(v.r[15])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld16(TRaw16 &a, TRaw16 &b, TRaw16 &c)
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(a.r[0]), "+r"(a.r[1]), "+r"(a.r[2]), "+r"(a.r[3]), "+r"(a.r[4]), "+r"(a.r[5]), "+r"(a.r[6]), "+r"(a.r[7]),
+                   "+r"(a.r[8]), "+r"(a.r[9]), "+r"(a.r[10]), "+r"(a.r[11]), "+r"(a.r[12]), "+r"(a.r[13]), "+r"(a.r[14]), "+r"(a.r[15]),
+                   "+r"(b.r[0]), "+r"(b.r[1]), "+r"(b.r[2]), "+r"(b.r[3]), "+r"(b.r[4]), "+r"(b.r[5]), "+r"(b.r[6]), "+r"(b.r[7]),
+                   "+r"(b.r[8]), "+r"(b.r[9]), "+r"(b.r[10]), "+r"(b.r[11]), "+r"(b.r[12]), "+r"(b.r[13]), "+r"(b.r[14]), "+r"(b.r[15]),
+                   "+r"(c.r[0]), "+r"(c.r[1]), "+r"(c.r[2]), "+r"(c.r[3]), "+r"(c.r[4]), "+r"(c.r[5]), "+r"(c.r[6]), "+r"(c.r[7]),
+                   "+r"(c.r[8]), "+r"(c.r[9]), "+r"(c.r[10]), "+r"(c.r[11]), "+r"(c.r[12]), "+r"(c.r[13]), "+r"(c.r[14]), "+r"(c.r[15])
+                 :: "memory");
+}
+__device__ __forceinline__ double traw16(const TRaw16 &v, int n) { return __hiloint2double((int)v.r[2 * n + 1], (int)v.r[2 * n]); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ double traw(const TRaw8 &v, int n) { return __hiloint2double((int)v.r[2 * n + 1], (int)v.r[2 * n]); }
 
@@ -513,7 +535,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                 if (lane == 0) u = 0.0;
             } else {
                 // ---- level 2: PCR over lanes 0..30; lane 31 is the warp's separator
-                const Row3 rp = pcr_lanes_0_30_rolled(row, lane);
+                const Row3 rp = (NW == 16) ? pcr_lanes_0_30(row, lane) : pcr_lanes_0_30_rolled(row, lane);
                 Row3 r30;
                 r30.a = __shfl_sync(FULL, rp.a, 30);
                 r30.c = __shfl_sync(FULL, rp.c, 30);
@@ -590,19 +612,18 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             double xn = y; // x_{k+1}
 #pragma unroll
             for (int hh = 1; hh >= 0; --hh) {
-                TRaw8 cr[6];
+                TRaw16 cr[3];
 #pragma unroll
-                for (int n = 0; n < 6; ++n) tmem_ld8(tm + (uint32_t)(48 * hh + 8 * n), cr[n]);
-                tmem_wait_ld3(cr[0], cr[1], cr[2]);
-                tmem_wait_ld3(cr[3], cr[4], cr[5]);
+                for (int n = 0; n < 3; ++n) tmem_ld16(tm + (uint32_t)(48 * hh + 16 * n), cr[n]);
+                tmem_wait_ld16(cr[0], cr[1], cr[2]);
                 double xs[8];
 #pragma unroll
                 for (int r = 7; r >= 0; --r) {
                     // row k = 8 hh + r: its (al, be, gm) are doubles 3r, 3r+1, 3r+2 of the 24 loaded
                     const int k = 8 * hh + r;
-                    const double a_ = traw(cr[(3 * r) >> 2], (3 * r) & 3);
-                    const double b_ = traw(cr[(3 * r + 1) >> 2], (3 * r + 1) & 3);
-                    const double g_ = traw(cr[(3 * r + 2) >> 2], (3 * r + 2) & 3);
+                    const double a_ = traw16(cr[(3 * r) >> 3], (3 * r) & 7);
+                    const double b_ = traw16(cr[(3 * r + 1) >> 3], (3 * r + 1) & 7);
+                    const double g_ = traw16(cr[(3 * r + 2) >> 3], (3 * r + 2) & 7);
                     xs[r] = (k == 15) ? y : fma(a_, xn, fma(g_, u, b_));
                     xn = xs[r];
                 }
