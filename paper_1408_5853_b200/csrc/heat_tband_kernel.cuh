@@ -121,6 +121,42 @@ __device__ __forceinline__ double traw(const TRaw8 &v, int n) { return __hiloint
 __device__ __forceinline__ constexpr uint32_t tcol_coef(int g, int part) { return (uint32_t)(24 * g + 8 * part); }
 __device__ __forceinline__ constexpr uint32_t tcol_flux(int g) { return (uint32_t)(96 + 8 * g); }
 
+// PCR elimination as pcr_combine (heat_line_kernel.cuh), with the boundary handled by masking the ONE
+// coefficient that does the elimination (a where there is no left row, c where there is no right row)
+// instead of the two values it would multiply: four selects fewer per step, same bits for finite rows
+// (-0 * x = -0, and 1 + -0 = 1, d + -0 = d exactly).
+__device__ __forceinline__ Row3 tpcr_combine(const Row3 &me, const Row3 &L, bool vl, const Row3 &R, bool vr)
+{
+    const double ae = vl ? me.a : 0.0, ce = vr ? me.c : 0.0;
+    double den = fma(-ae, L.c, 1.0);
+    den = fma(-ce, R.a, den);
+    const double r = rcp_cubic(den);
+    double d = fma(-ae, L.d, me.d);
+    d = fma(-ce, R.d, d);
+    Row3 o;
+    o.d = d * r;
+    const double ar_ = me.a * r, cr_ = me.c * r;
+    o.a = vl ? -ar_ * L.a : ar_; // an external reference keeps its coefficient
+    o.c = vr ? -cr_ * R.c : cr_;
+    return o;
+}
+template <bool UNROLL>
+__device__ __forceinline__ Row3 tpcr_lanes_0_30(Row3 row, int lane)
+{
+#pragma unroll (UNROLL ? 5 : 1)
+    for (int s = 1; s < 32; s <<= 1) {
+        Row3 L, R;
+        L.a = __shfl_up_sync(0xffffffffu, row.a, s);
+        L.c = __shfl_up_sync(0xffffffffu, row.c, s);
+        L.d = __shfl_up_sync(0xffffffffu, row.d, s);
+        R.a = __shfl_down_sync(0xffffffffu, row.a, s);
+        R.c = __shfl_down_sync(0xffffffffu, row.c, s);
+        R.d = __shfl_down_sync(0xffffffffu, row.d, s);
+        row = tpcr_combine(row, L, lane >= s, R, lane + s <= 30);
+    }
+    return row;
+}
+
 struct TSweepArgs {
     uint32_t sc, su;         // shared addresses: line j, line j+1
     uint32_t tm;             // tensor-memory address of the warp's strip (column 0)
@@ -535,7 +571,7 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
                 if (lane == 0) u = 0.0;
             } else {
                 // ---- level 2: PCR over lanes 0..30; lane 31 is the warp's separator
-                const Row3 rp = (NW == 16) ? pcr_lanes_0_30(row, lane) : pcr_lanes_0_30_rolled(row, lane);
+                const Row3 rp = tpcr_lanes_0_30<NW == 16>(row, lane);
                 Row3 r30;
                 r30.a = __shfl_sync(FULL, rp.a, 30);
                 r30.c = __shfl_sync(FULL, rp.c, 30);
