@@ -140,8 +140,10 @@ __device__ __forceinline__ Row3 tpcr_combine(const Row3 &me, const Row3 &L, bool
     o.c = vr ? -cr_ * R.c : cr_;
     return o;
 }
-template <bool UNROLL>
-__device__ __forceinline__ Row3 tpcr_lanes_0_30(Row3 row, int lane)
+// HI = 30: PCR over lanes 0..30 (lane 31, the warp's separator, runs along and produces values nobody reads);
+// HI = 31: over the whole warp (a line of one warp).
+template <bool UNROLL, int HI>
+__device__ __forceinline__ Row3 tpcr_lanes(Row3 row, int lane)
 {
 #pragma unroll (UNROLL ? 5 : 1)
     for (int s = 1; s < 32; s <<= 1) {
@@ -152,7 +154,7 @@ __device__ __forceinline__ Row3 tpcr_lanes_0_30(Row3 row, int lane)
         R.a = __shfl_down_sync(0xffffffffu, row.a, s);
         R.c = __shfl_down_sync(0xffffffffu, row.c, s);
         R.d = __shfl_down_sync(0xffffffffu, row.d, s);
-        row = tpcr_combine(row, L, lane >= s, R, lane + s <= 30);
+        row = tpcr_combine(row, L, lane >= s, R, lane + s <= HI);
     }
     return row;
 }
@@ -565,13 +567,13 @@ __global__ void __launch_bounds__(32 * NW, 16 / NW) heat_tband_kernel(const __gr
             double y, u;
             if constexpr (WL == 1) {
                 // the whole line is this warp: PCR over all 32 reduced rows
-                row = pcr_segment_rolled<32>(row, lane, 0, 31);
+                row = tpcr_lanes<false, 31>(row, lane);
                 y = row.d;
                 u = __shfl_up_sync(FULL, y, 1);
                 if (lane == 0) u = 0.0;
             } else {
                 // ---- level 2: PCR over lanes 0..30; lane 31 is the warp's separator
-                const Row3 rp = tpcr_lanes_0_30<NW == 16>(row, lane);
+                const Row3 rp = tpcr_lanes<NW == 16, 30>(row, lane);
                 Row3 r30;
                 r30.a = __shfl_sync(FULL, rp.a, 30);
                 r30.c = __shfl_sync(FULL, rp.c, 30);
