@@ -32,7 +32,7 @@ BYTES_PER_CELL = 16.0  # algorithmic: 8 B read of T^k + 8 B write of T^{k+1} (DE
 # fp64 thread-instructions (DFMA + DMUL + DADD) per cell-update, by kernel family, from the ncu counters
 # smsp__sass_thread_inst_executed_op_d{fma,mul,add}_pred_on of the committed captures (profiles/*.md name
 # them); a kernel without an entry gets no `roofline_alu` object rather than a guessed one
-FP64_PER_CELL = {"tband<WL=16": 40.8, "band<G=256,CL=4": 48.0}
+FP64_PER_CELL = {"tband<WL=16": 40.1, "band<G=256,CL=4": 48.0}
 FP64_LANES = 148 * 64  # fp64 lanes of a B200 (64 per SM): the nominal ALU peak stated beside the measured one
 
 

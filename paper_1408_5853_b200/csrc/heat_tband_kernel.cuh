@@ -128,11 +128,13 @@ __device__ __forceinline__ constexpr uint32_t tcol_flux(int g) { return (uint32_
 __device__ __forceinline__ Row3 tpcr_combine(const Row3 &me, const Row3 &L, bool vl, const Row3 &R, bool vr)
 {
     const double ae = vl ? me.a : 0.0, ce = vr ? me.c : 0.0;
-    double den = fma(-ae, L.c, 1.0);
-    den = fma(-ce, R.a, den);
+    // (the minus sign on the shuffled operand: it is an operand modifier there, whereas negating the
+    // selected ae / ce would cost an instruction on the FP64 pipe; the products are the same bits)
+    double den = fma(ae, -L.c, 1.0);
+    den = fma(ce, -R.a, den);
     const double r = rcp_cubic(den);
-    double d = fma(-ae, L.d, me.d);
-    d = fma(-ce, R.d, d);
+    double d = fma(ae, -L.d, me.d);
+    d = fma(ce, -R.d, d);
     Row3 o;
     o.d = d * r;
     const double ar_ = me.a * r, cr_ = me.c * r;
